@@ -1,0 +1,124 @@
+/*
+ * gce_ce.h -- C ABI of the B200-native Conditional Entropy (P, Pdot) period search.
+ *
+ * What the library computes (Katz et al., arXiv 2006.06866; citations are lines of PAPER.md):
+ *   for every light curve and every trial (P, Pdot) of a caller-supplied grid
+ *     S1  normalise: t0 = min t, magnitudes min/max-scaled to [0,1], magnitude bin per point   (:96)
+ *     S2  fold each time to a phase that includes the Pdot term, Eq. 3                          (:100-102)
+ *     S3  bin the points into an n_phase x n_mag histogram                                      (:106)
+ *     S4  CE = sum_ij p(m_i,phi_j) ln( p(phi_j) / p(m_i,phi_j) ), Eq. 4                         (:108-110)
+ *     S5  store CE and/or select the k smallest per light curve (minimum = best period)         (:49, :112)
+ *   optionally the significance statistics of Eq. 5 (:112-116).
+ * The arithmetic (operation order of the fp64 fold, bin edge ownership, tie rule) is frozen in
+ * DESIGN.md section 3; histogram counts and bin indices are bit-exact against that definition.
+ *
+ * Conventions
+ *   - Plain C types only.  Pointers are DEVICE pointers unless the parameter name ends in _host or the
+ *     function name ends in _host.  All arrays are caller-owned; the library never frees or retains them.
+ *   - gce_ce_search and the debug calls only enqueue work on `stream` (a cudaStream_t passed as void*,
+ *     NULL = default stream) and return without synchronising; results are valid once the stream has
+ *     reached that point.  gce_ce_search_host synchronises before returning.
+ *   - Return value: 0 (GCE_CE_OK) = enqueued; negative = error and nothing was enqueued.
+ *   - No global mutable state; re-entrant across streams as long as each call has its own workspace.
+ *   - `times` need not be sorted.  `periods` are in the unit of `times`; `pdots` are dimensionless (s/s), any
+ *     sign (:228).  Trials are addressed by the flat index q = ip * n_pdot + ipd.
+ *   - Values that need device data to validate (non-monotone lc_offsets, P <= 0, non-finite inputs, a light
+ *     curve longer than GCE_CE_MAX_POINTS) are undefined behaviour; gce_ce_validate_host checks host copies.
+ *   - A light curve with N = 0 yields CE = NaN for every trial and best index -1; N = 1 yields CE = 0.
+ *   - There is no CPU fallback anywhere in this library.
+ */
+#ifndef GCE_CE_H_
+#define GCE_CE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GCE_CE_OK 0
+#define GCE_CE_ERR_POINTER (-1)   /* NULL / inconsistent pointer combination                       */
+#define GCE_CE_ERR_RANGE (-2)     /* a size or bin count is out of range                           */
+#define GCE_CE_ERR_WORKSPACE (-3) /* workspace too small or misaligned                             */
+#define GCE_CE_ERR_CUDA (-4)      /* a CUDA runtime call failed; see gce_ce_last_cuda_error()       */
+
+#define GCE_CE_MAX_BINS 64         /* n_phase_bins and n_mag_bins are each in 1..64                 */
+#define GCE_CE_MAX_TOPK 32         /* top_k is in 0..32                                             */
+#define GCE_CE_MAX_POINTS 65535    /* points per light curve (16-bit counters)                      */
+
+typedef struct gce_ce_params {
+    int32_t n_phase_bins; /* n_phi, 1..64                                                         */
+    int32_t n_mag_bins;   /* n_m,   1..64                                                         */
+    int32_t top_k;        /* 0 = no selection output; 1..32 = keep the k smallest CE per LC        */
+    int32_t ce_fp64;      /* 0: out_ce is float[...]; 1: out_ce is double[...]                     */
+    int32_t want_stats;   /* 1: out_stats receives the Eq. 5 statistics (requires out_stats)      */
+    int32_t overlap;      /* 0: plain bins (hot path).  1: 50 % overlapping phase bins (:106, N2)  */
+    int32_t reserved[2];  /* must be 0                                                            */
+} gce_ce_params;
+
+/* Bytes of device workspace gce_ce_search needs for these sizes (256-byte aligned base required).
+ * total_points = lc_offsets[n_lc] (the caller knows it on the host). */
+int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int64_t n_pdot,
+                           const gce_ce_params *prm_host, size_t *bytes_host);
+
+/*
+ * The search (S1..S5).  Layouts:
+ *   times, mags      double[total_points], light curves back to back (CSR)
+ *   lc_offsets       int64[n_lc + 1], lc_offsets[0] = 0, non-decreasing
+ *   periods          double[n_p], pdots double[n_pdot]
+ *   out_ce           NULL, or [n_lc][n_p][n_pdot] (Pdot fastest) float or double per prm->ce_fp64
+ *   out_best_idx     NULL (iff top_k == 0), or int64[n_lc][top_k]: flat q of the k smallest CE, ascending by
+ *                    (CE, q); -1 where fewer than k trials exist or N = 0
+ *   out_best_ce      NULL, or float[n_lc][top_k] matching out_best_idx (NaN where idx = -1)
+ *   out_stats        NULL, or double[n_lc][4] = {mean CE, population std, min CE, rho = (mean-min)/std}
+ *                    over all trials of the light curve (Eq. 5)
+ * At least one of out_ce / out_best_idx / out_stats must be non-NULL.
+ */
+int gce_ce_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                  int64_t total_points, const double *periods, int64_t n_p, const double *pdots,
+                  int64_t n_pdot, const gce_ce_params *prm_host, void *out_ce, int64_t *out_best_idx,
+                  float *out_best_ce, double *out_stats, void *workspace, size_t workspace_bytes,
+                  void *stream);
+
+/* Same call with HOST buffers for every array: allocates device memory, copies inputs in, runs the
+ * search, copies the requested outputs back and synchronises.  Convenience / end-to-end timing entry. */
+int gce_ce_search_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                       const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                       const gce_ce_params *prm_host, void *out_ce, int64_t *out_best_idx,
+                       float *out_best_ce, double *out_stats);
+
+/* Test-only: the production search kernel run in "dump" mode over a list of flat trial indices
+ * (device int64[n_trials], the same list for every light curve); writes the histogram counts
+ *   out_counts uint32[n_lc][n_trials][n_phase_bins][n_mag_bins]      (phase-major, as Eq. 4's n_ij)
+ * and, if out_ce_at != NULL, double[n_lc][n_trials] CE of those trials. */
+int gce_ce_debug_histogram(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                           int64_t total_points, const double *periods, int64_t n_p, const double *pdots,
+                           int64_t n_pdot, const gce_ce_params *prm_host, const int64_t *trial_q,
+                           int64_t n_trials, uint32_t *out_counts, double *out_ce_at, void *workspace,
+                           size_t workspace_bytes, void *stream);
+
+/* Test-only: phase bin and magnitude bin of every point of light curve `lc` for trial q, in the caller's
+ * point order: out_phase_bin int32[N], out_mag_bin int32[N]. */
+int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                      const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                      const gce_ce_params *prm_host, int32_t lc, int64_t q, int32_t *out_phase_bin,
+                      int32_t *out_mag_bin, void *stream);
+
+/* Synchronous argument checker on HOST copies of the arrays (the hot call never synchronises).
+ * Returns GCE_CE_OK or the first error found. */
+int gce_ce_validate_host(const double *times_host, const double *mags_host, const int64_t *lc_offsets_host,
+                         int32_t n_lc, const double *periods_host, int64_t n_p, const double *pdots_host,
+                         int64_t n_pdot, const gce_ce_params *prm_host);
+
+/* Number of kernels one gce_ce_search call enqueues for these arguments (for launch accounting). */
+int gce_ce_launch_count(int32_t n_lc, const gce_ce_params *prm_host);
+
+const char *gce_ce_strerror(int code);
+int gce_ce_last_cuda_error(void); /* cudaError_t of the most recent GCE_CE_ERR_CUDA on this thread */
+const char *gce_ce_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GCE_CE_H_ */

@@ -1,0 +1,233 @@
+"""Thin ctypes binding of include/gce_ce.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libgce_ce.so.  PyTorch is used for device memory and
+the stream handle; nothing here computes.  There is no CPU fallback: if the library has not been built
+(`python -m paper_2006_06866_b200.build`) importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from .build import LIB
+
+if not os.path.exists(LIB):
+    raise ImportError(f"{LIB} is missing: run `python -m paper_2006_06866_b200.build` (nvcc, sm_100a). "
+                      "There is no CPU fallback.")
+
+_lib = C.CDLL(LIB)
+
+MAX_BINS, MAX_TOPK, MAX_POINTS = 64, 32, 65535
+OK, ERR_POINTER, ERR_RANGE, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
+
+
+class Params(C.Structure):
+    _fields_ = [("n_phase_bins", C.c_int32), ("n_mag_bins", C.c_int32), ("top_k", C.c_int32),
+                ("ce_fp64", C.c_int32), ("want_stats", C.c_int32), ("overlap", C.c_int32),
+                ("reserved", C.c_int32 * 2)]
+
+
+_vp, _i32, _i64, _sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
+_lib.gce_ce_workspace_bytes.argtypes = [_i64, _i32, _i64, _i64, C.POINTER(Params), C.POINTER(_sz)]
+_lib.gce_ce_search.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params),
+                               _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.gce_ce_search_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _vp, _vp, _vp, _vp]
+_lib.gce_ce_debug_histogram.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params),
+                                        _vp, _i64, _vp, _vp, _vp, _sz, _vp]
+_lib.gce_ce_debug_bins.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _i32, _i64,
+                                   _vp, _vp, _vp]
+_lib.gce_ce_validate_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params)]
+_lib.gce_ce_launch_count.argtypes = [_i32, C.POINTER(Params)]
+_lib.gce_ce_strerror.argtypes = [C.c_int]
+_lib.gce_ce_strerror.restype = C.c_char_p
+_lib.gce_ce_version.restype = C.c_char_p
+for _f in ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
+           "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_last_cuda_error"):
+    getattr(_lib, _f).restype = C.c_int
+
+EXPORTS = ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
+           "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_strerror",
+           "gce_ce_last_cuda_error", "gce_ce_version")
+
+
+class GceError(RuntimeError):
+    def __init__(self, code):
+        self.code = int(code)
+        msg = _lib.gce_ce_strerror(self.code).decode()
+        if self.code == ERR_CUDA:
+            msg += f" [cudaError {_lib.gce_ce_last_cuda_error()}]"
+        super().__init__(f"gce_ce error {self.code}: {msg}")
+
+
+def _check(rc):
+    if rc != OK:
+        raise GceError(rc)
+
+
+def gce_ce_version() -> str:
+    return _lib.gce_ce_version().decode()
+
+
+def make_params(n_phase_bins, n_mag_bins, top_k=0, ce_fp64=False, want_stats=False, overlap=False) -> Params:
+    return Params(int(n_phase_bins), int(n_mag_bins), int(top_k), int(bool(ce_fp64)), int(bool(want_stats)),
+                  int(bool(overlap)), (C.c_int32 * 2)(0, 0))
+
+
+def gce_ce_workspace_bytes(total_points, n_lc, n_p, n_pdot, prm: Params) -> int:
+    out = _sz(0)
+    _check(_lib.gce_ce_workspace_bytes(int(total_points), int(n_lc), int(n_p), int(n_pdot), C.byref(prm), C.byref(out)))
+    return int(out.value)
+
+
+def gce_ce_launch_count(n_lc, prm: Params) -> int:
+    return int(_lib.gce_ce_launch_count(int(n_lc), C.byref(prm)))
+
+
+def _dev(t, dtype):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"expected a contiguous CUDA tensor of {dtype}")
+    return t
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def gce_ce_search(times, mags, lc_offsets, periods, pdots, prm: Params, out_ce=None, out_best_idx=None,
+                  out_best_ce=None, out_stats=None, workspace=None, stream=None):
+    """Enqueue the search on `stream` (default: torch's current stream).  All tensors are CUDA tensors the caller
+    owns; see include/gce_ce.h for layouts.  Returns nothing; outputs are the tensors passed in."""
+    times, mags = _dev(times, torch.float64), _dev(mags, torch.float64)
+    lc_offsets = _dev(lc_offsets, torch.int64)
+    periods, pdots = _dev(periods, torch.float64), _dev(pdots, torch.float64)
+    n_lc = lc_offsets.numel() - 1
+    ce_dtype = torch.float64 if prm.ce_fp64 else torch.float32
+    if out_ce is not None:
+        _dev(out_ce, ce_dtype)
+        if out_ce.numel() != n_lc * periods.numel() * pdots.numel():
+            raise ValueError("out_ce has the wrong number of elements")
+    if out_best_idx is not None:
+        _dev(out_best_idx, torch.int64)
+        if out_best_idx.numel() != n_lc * prm.top_k:
+            raise ValueError("out_best_idx has the wrong number of elements")
+    if out_best_ce is not None:
+        _dev(out_best_ce, torch.float32)
+        if out_best_ce.numel() != n_lc * prm.top_k:
+            raise ValueError("out_best_ce has the wrong number of elements")
+    if out_stats is not None:
+        _dev(out_stats, torch.float64)
+    if workspace is None or not workspace.is_cuda:
+        raise TypeError("workspace must be a CUDA tensor (see gce_ce_workspace_bytes)")
+    _check(_lib.gce_ce_search(_ptr(times), _ptr(mags), _ptr(lc_offsets), n_lc, times.numel(), _ptr(periods),
+                              periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), _ptr(out_ce),
+                              _ptr(out_best_idx), _ptr(out_best_ce), _ptr(out_stats), _ptr(workspace),
+                              workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def gce_ce_debug_histogram(times, mags, lc_offsets, periods, pdots, prm: Params, trial_q, out_counts, out_ce_at=None,
+                           workspace=None, stream=None):
+    n_lc = lc_offsets.numel() - 1
+    _dev(trial_q, torch.int64)
+    _dev(out_counts, torch.int32)  # uint32 counts viewed as int32 storage
+    if out_counts.numel() != n_lc * trial_q.numel() * prm.n_phase_bins * prm.n_mag_bins:
+        raise ValueError("out_counts has the wrong number of elements")
+    if out_ce_at is not None:
+        _dev(out_ce_at, torch.float64)
+    _check(_lib.gce_ce_debug_histogram(_ptr(times), _ptr(mags), _ptr(lc_offsets), n_lc, times.numel(), _ptr(periods),
+                                       periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), _ptr(trial_q),
+                                       trial_q.numel(), _ptr(out_counts), _ptr(out_ce_at), _ptr(workspace),
+                                       workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def gce_ce_debug_bins(times, mags, lc_offsets, periods, pdots, prm: Params, lc, q, out_phase_bin, out_mag_bin,
+                      stream=None):
+    n_lc = lc_offsets.numel() - 1
+    _dev(out_phase_bin, torch.int32)
+    _dev(out_mag_bin, torch.int32)
+    _check(_lib.gce_ce_debug_bins(_ptr(times), _ptr(mags), _ptr(lc_offsets), n_lc, _ptr(periods), periods.numel(),
+                                  _ptr(pdots), pdots.numel(), C.byref(prm), int(lc), int(q), _ptr(out_phase_bin),
+                                  _ptr(out_mag_bin), _stream(stream)))
+
+
+def _host(a, dtype):
+    """Host buffer -> (object keeping it alive, address).  Accepts numpy arrays and (pinned) CPU torch tensors."""
+    if a is None:
+        return None, None
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or not a.is_contiguous():
+            raise TypeError("expected a contiguous CPU tensor")
+        return a, C.c_void_p(a.data_ptr())
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a, C.c_void_p(a.ctypes.data)
+
+
+def gce_ce_search_host(times, mags, lc_offsets, periods, pdots, prm: Params, out_ce=None, out_best_idx=None,
+                       out_best_ce=None, out_stats=None):
+    """Same call with HOST buffers (numpy or CPU torch tensors); copies in, runs, copies out, synchronises."""
+    keep = []
+    ptrs = []
+    for a, dt in ((times, np.float64), (mags, np.float64), (lc_offsets, np.int64), (periods, np.float64),
+                  (pdots, np.float64)):
+        k, p = _host(a, dt)
+        keep.append(k)
+        ptrs.append(p)
+    n_lc = (keep[2].numel() if isinstance(keep[2], torch.Tensor) else keep[2].shape[0]) - 1
+    n_p = keep[3].numel() if isinstance(keep[3], torch.Tensor) else keep[3].shape[0]
+    n_pdot = keep[4].numel() if isinstance(keep[4], torch.Tensor) else keep[4].shape[0]
+    outs = []
+    for a in (out_ce, out_best_idx, out_best_ce, out_stats):
+        if a is None:
+            outs.append(None)
+        elif isinstance(a, torch.Tensor):
+            outs.append(C.c_void_p(a.data_ptr()))
+        else:
+            if not a.flags["C_CONTIGUOUS"]:
+                raise TypeError("output arrays must be C-contiguous")
+            outs.append(C.c_void_p(a.ctypes.data))
+    _check(_lib.gce_ce_search_host(ptrs[0], ptrs[1], ptrs[2], n_lc, ptrs[3], n_p, ptrs[4], n_pdot, C.byref(prm),
+                                   outs[0], outs[1], outs[2], outs[3]))
+
+
+def gce_ce_validate_host(times, mags, lc_offsets, periods, pdots, prm: Params) -> int:
+    t, m = np.ascontiguousarray(times, np.float64), np.ascontiguousarray(mags, np.float64)
+    o = np.ascontiguousarray(lc_offsets, np.int64)
+    p, pd = np.ascontiguousarray(periods, np.float64), np.ascontiguousarray(pdots, np.float64)
+    return int(_lib.gce_ce_validate_host(C.c_void_p(t.ctypes.data), C.c_void_p(m.ctypes.data), C.c_void_p(o.ctypes.data),
+                                         o.shape[0] - 1, C.c_void_p(p.ctypes.data), p.shape[0],
+                                         C.c_void_p(pd.ctypes.data), pd.shape[0], C.byref(prm)))
+
+
+# ------------------------------------------------------------------------------------------ convenience
+class SearchResult:
+    __slots__ = ("ce", "best_idx", "best_ce", "stats")
+
+    def __init__(self, ce, best_idx, best_ce, stats):
+        self.ce, self.best_idx, self.best_ce, self.stats = ce, best_idx, best_ce, stats
+
+
+def search(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, top_k=0, want_cube=True,
+           ce_fp64=False, want_stats=False, overlap=False, workspace=None, stream=None) -> SearchResult:
+    """Allocate outputs + workspace with torch and call gce_ce_search (device tensors in, device tensors out)."""
+    prm = make_params(n_phase_bins, n_mag_bins, top_k, ce_fp64, want_stats, overlap)
+    dev = times.device
+    n_lc = lc_offsets.numel() - 1
+    n_p, n_pdot = periods.numel(), pdots.numel()
+    ce = torch.empty((n_lc, n_p, n_pdot), dtype=torch.float64 if ce_fp64 else torch.float32, device=dev) if want_cube else None
+    bidx = torch.empty((n_lc, top_k), dtype=torch.int64, device=dev) if top_k > 0 else None
+    bce = torch.empty((n_lc, top_k), dtype=torch.float32, device=dev) if top_k > 0 else None
+    stats = torch.empty((n_lc, 4), dtype=torch.float64, device=dev) if want_stats else None
+    if workspace is None:
+        nbytes = gce_ce_workspace_bytes(times.numel(), n_lc, n_p, n_pdot, prm)
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    gce_ce_search(times, mags, lc_offsets, periods, pdots, prm, ce, bidx, bce, stats, workspace, stream)
+    return SearchResult(ce, bidx, bce, stats)

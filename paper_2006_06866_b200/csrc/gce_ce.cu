@@ -1,0 +1,944 @@
+// gce_ce.cu -- B200 (sm_100a) kernels and C ABI of the Conditional Entropy (P, Pdot) search.
+//
+// Path (citations are PAPER.md lines of arXiv 2006.06866):
+//   k_preprocess  S1  t0 / min-max / magnitude bin per point, points grouped by magnitude bin      (:96)
+//   k_ltab            fixed-point table L(k) = k ln k used by S4
+//   k_search      S2  fp64 fold, Eq. 3, frozen operation order               (:100)
+//                 S3  per-trial private histogram in shared memory                                 (:106)
+//                 S4  N*CE = sum_j L(n_j) - sum_ij L(n_ij), exact integer accumulation, Eq. 4      (:108)
+//                 S5  CE cube store + per-warp running top-k                                       (:49, :112)
+//   k_merge_topk  S5  per-light-curve merge of the per-CTA candidates
+//
+// Design (B200-first): one THREAD owns R consecutive trials (the paper's one-thread-
+// per-grid-point idea, :152, kept because it makes every shared-memory access conflict-free), the light curve
+// is streamed through a small ring of shared-memory stages by TMA bulk copies (cp.async.bulk + mbarrier) and
+// is shared by every thread of the CTA (broadcast LDS.128), points are pre-grouped by magnitude bin so a trial
+// only needs a 1-D phase histogram at a time (the paper's memory insight, :152), counters are 16-bit pairs in
+// a [bin][thread] column layout (bank = lane), and the entropy is accumulated in 2^-42 fixed point so CE does
+// not depend on summation order.  No tensor cores: this is a histogram/entropy path, not a contraction.
+//
+// This translation unit must be compiled with -fmad=false; the fold additionally uses explicit _rn/_rd
+// intrinsics, which are never contracted.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+#include <string.h>
+
+#include "gce_ce.h"
+
+#ifndef GCE_HIST_ATOMIC
+#define GCE_HIST_ATOMIC 1 /* 1: ATOMS.ADD without return; 0: LDS + IADD + STS (thread-private, race-free) */
+#endif
+
+namespace {
+
+constexpr int kChunk = 512;       // points per shared-memory stage (16 B each -> 8 KB)
+constexpr int kStages = 3;        // TMA ring depth
+constexpr int kUnroll = 2;        // points loaded ahead per thread in the hot loop
+constexpr int kLtabSmem = 1024;   // entries of the L table mirrored in shared memory
+constexpr int kLfixShift = 42;    // L table fixed point: 2^-42
+constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(y) in the low mantissa word
+constexpr int64_t kInfS = INT64_MAX;
+
+struct LcInfo {
+    int32_t n;
+    int32_t pad;
+    double dt_max;
+};
+
+struct SearchParams {
+    const double2 *pts;        // [total_points] (dt, dt2), grouped by magnitude bin inside each light curve
+    const int32_t *seg;        // [n_lc][n_m + 1] segment offsets relative to the light curve start
+    const LcInfo *info;        // [n_lc]
+    const int64_t *lc_offsets; // [n_lc + 1]
+    const int64_t *ltab;       // [ltab_n] fixed-point k ln k
+    const double *periods;
+    const double *pdots;
+    const int64_t *trial_q;    // DUMP only
+    int64_t n_p, n_pdot, n_trials;
+    int64_t tiles_per_lc;
+    int32_t jobs_per_lc;
+    int32_t n_phi, n_m;
+    uint32_t mod_mul, mod_bias;
+    double y_safe;             // |y| below this -> 32-bit fast floor/mod path is exact
+    int32_t ltab_n;
+    int32_t top_k;
+    int32_t ce_fp64;
+    void *out_ce;              // cube or NULL
+    int64_t *part_S, *part_q;  // [n_lc][jobs_per_lc][top_k]
+    uint32_t *out_counts;      // DUMP only
+    double *out_ce_at;         // DUMP only
+};
+
+// ------------------------------------------------------------------------------------------------ helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void tma_load_bulk(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// (S, q) lexicographic order: exact integer N*CE first, then flat trial index (tie rule Q9).
+__device__ __forceinline__ bool key_less(int64_t s1, int64_t q1, int64_t s2, int64_t q2) {
+    return (s1 < s2) || (s1 == s2 && q1 < q2);
+}
+
+// Warp-distributed sorted list: lane l holds the l-th best (S, q); lanes >= k hold +inf.
+struct WarpTopK {
+    int64_t S, q;       // this lane's element
+    int64_t thrS, thrq; // the k-th (worst kept) element, replicated
+    int k;
+    __device__ __forceinline__ void reset(int k_) {
+        k = k_;
+        S = kInfS; q = kInfS; thrS = kInfS; thrq = kInfS;
+    }
+    // Every lane offers one candidate (cS = kInfS for "none"); warp-uniform call.
+    __device__ __forceinline__ void offer(int64_t cS, int64_t cq) {
+        const int lane = threadIdx.x & 31;
+        unsigned mask = __ballot_sync(0xffffffffu, key_less(cS, cq, thrS, thrq));
+        while (mask) {
+            const int src = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const int64_t xS = __shfl_sync(0xffffffffu, cS, src);
+            const int64_t xq = __shfl_sync(0xffffffffu, cq, src);
+            if (!key_less(xS, xq, thrS, thrq)) continue;  // threshold moved since the ballot
+            const int pos = __popc(__ballot_sync(0xffffffffu, key_less(S, q, xS, xq)));
+            const int64_t upS = __shfl_up_sync(0xffffffffu, S, 1);
+            const int64_t upq = __shfl_up_sync(0xffffffffu, q, 1);
+            if (lane == pos) { S = xS; q = xq; }
+            else if (lane > pos) { S = upS; q = upq; }
+            if (lane >= k) { S = kInfS; q = kInfS; }
+            thrS = __shfl_sync(0xffffffffu, S, k - 1);
+            thrq = __shfl_sync(0xffffffffu, q, k - 1);
+        }
+    }
+};
+
+// S1 magnitude bin: min(floor(((m - m_lo) / r) * n_m), n_m - 1); r == 0 -> 0.
+__device__ __forceinline__ int mag_bin(double m, double m_lo, double r, int n_m) {
+    if (r == 0.0) return 0;
+    const double u = __ddiv_rn(__dsub_rn(m, m_lo), r);
+    const int i = __double2int_rd(__dmul_rn(u, (double)n_m));
+    return i < n_m - 1 ? i : n_m - 1;
+}
+
+// S2, slow generic form (any |y| < 2^62): exactly the listing of DESIGN.md section 3.
+__device__ __forceinline__ int fold_bin_generic(double dt, double dt2, double invP, double c, int n_phi) {
+    const double a = __dmul_rn(dt, invP);
+    const double b = __dmul_rn(dt2, c);
+    const double x = __dadd_rn(a, b);
+    const double y = __dmul_rn(x, (double)n_phi);
+    const long long I = __double2ll_rd(y);
+    long long j = I % (long long)n_phi;
+    if (j < 0) j += n_phi;
+    return (int)j;
+}
+
+__device__ __forceinline__ void trial_constants(double P, double Pdot, double &invP, double &c) {
+    invP = __ddiv_rn(1.0, P);
+    c = __dmul_rn(__dmul_rn(__dmul_rn(-0.5, Pdot), invP), invP);
+}
+
+struct MinMax3 {
+    double tmin, tmax, mmin, mmax;
+};
+
+__device__ __forceinline__ MinMax3 block_minmax(MinMax3 v, MinMax3 *sh) {
+    for (int o = 16; o > 0; o >>= 1) {
+        const double a = __shfl_xor_sync(0xffffffffu, v.tmin, o);
+        const double b = __shfl_xor_sync(0xffffffffu, v.tmax, o);
+        const double c = __shfl_xor_sync(0xffffffffu, v.mmin, o);
+        const double d = __shfl_xor_sync(0xffffffffu, v.mmax, o);
+        v.tmin = a < v.tmin ? a : v.tmin;
+        v.tmax = b > v.tmax ? b : v.tmax;
+        v.mmin = c < v.mmin ? c : v.mmin;
+        v.mmax = d > v.mmax ? d : v.mmax;
+    }
+    const int w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    if ((threadIdx.x & 31) == 0) sh[w] = v;
+    __syncthreads();
+    MinMax3 r = sh[0];
+    for (int i = 1; i < nw; ++i) {
+        r.tmin = sh[i].tmin < r.tmin ? sh[i].tmin : r.tmin;
+        r.tmax = sh[i].tmax > r.tmax ? sh[i].tmax : r.tmax;
+        r.mmin = sh[i].mmin < r.mmin ? sh[i].mmin : r.mmin;
+        r.mmax = sh[i].mmax > r.mmax ? sh[i].mmax : r.mmax;
+    }
+    __syncthreads();
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------------ S1
+// One CTA per light curve.  Output points are permuted so equal magnitude bins are contiguous (counts do not
+// depend on point order); seg[lc][i] is the first point of magnitude bin i, seg[lc][n_m] = N.
+__global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ times, const double *__restrict__ mags,
+                                                    const int64_t *__restrict__ lc_offsets, int n_m,
+                                                    double2 *__restrict__ pts, int32_t *__restrict__ seg,
+                                                    LcInfo *__restrict__ info) {
+    __shared__ MinMax3 sh_red[8];
+    __shared__ int sh_cnt[GCE_CE_MAX_BINS + 1];
+    __shared__ int sh_cur[GCE_CE_MAX_BINS];
+    const int lc = blockIdx.x;
+    const int64_t off = lc_offsets[lc];
+    const int n = (int)(lc_offsets[lc + 1] - off);
+    const double *t = times + off, *m = mags + off;
+
+    MinMax3 v{CUDART_INF, -CUDART_INF, CUDART_INF, -CUDART_INF};
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const double tk = t[k], mk = m[k];
+        v.tmin = tk < v.tmin ? tk : v.tmin;
+        v.tmax = tk > v.tmax ? tk : v.tmax;
+        v.mmin = mk < v.mmin ? mk : v.mmin;
+        v.mmax = mk > v.mmax ? mk : v.mmax;
+    }
+    v = block_minmax(v, sh_red);
+    const double t0 = v.tmin, m_lo = v.mmin, r = __dsub_rn(v.mmax, v.mmin);
+
+    for (int i = threadIdx.x; i <= n_m; i += blockDim.x) sh_cnt[i] = 0;
+    __syncthreads();
+    for (int k = threadIdx.x; k < n; k += blockDim.x) atomicAdd(&sh_cnt[mag_bin(m[k], m_lo, r, n_m)], 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int i = 0; i < n_m; ++i) {
+            const int c = sh_cnt[i];
+            seg[(int64_t)lc * (n_m + 1) + i] = acc;
+            sh_cur[i] = acc;
+            acc += c;
+        }
+        seg[(int64_t)lc * (n_m + 1) + n_m] = acc;
+        info[lc].n = n;
+        info[lc].pad = 0;
+        info[lc].dt_max = n > 0 ? __dsub_rn(v.tmax, t0) : 0.0;
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const int i = mag_bin(m[k], m_lo, r, n_m);
+        const int pos = atomicAdd(&sh_cur[i], 1);
+        const double dt = __dsub_rn(t[k], t0);
+        pts[off + pos] = make_double2(dt, __dmul_rn(dt, dt));
+    }
+}
+
+// L(k) = k ln k in 2^-42 fixed point (k < 2^16 -> L < 2^20, so sums of up to N entries fit in int64).
+__global__ void k_ltab(int64_t *__restrict__ ltab, int n) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) ltab[k] = k < 2 ? 0 : __double2ll_rn(ldexp((double)k * log((double)k), kLfixShift));
+}
+
+// ------------------------------------------------------------------------------------------------ S2..S5
+// R = trials per thread (1, 2 or 4).  SHARE_P: the R trials of a thread share one period (n_pdot % R == 0), so
+// a = dt * invP is computed once (bit-identical: a does not depend on Pdot).  DUMP: test mode, trials come from
+// a list and the count tables are written out.
+template <int R, bool SHARE_P, bool DUMP>
+__global__ void __launch_bounds__(1024, 1) k_search(const SearchParams prm) {
+    constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int NT = blockDim.x, NW = NT >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int n_phi = prm.n_phi, n_m = prm.n_m;
+
+    // shared-memory carve-up
+    double2 *spts = reinterpret_cast<double2 *>(smem_raw);                                    // [kStages][kChunk]
+    int64_t *sL = reinterpret_cast<int64_t *>(spts + kStages * kChunk);                       // [kLtabSmem]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);                            // [kStages]
+    int *done = reinterpret_cast<int *>(full + kStages);                                      // [kStages]
+    int *sseg = done + kStages + 1;                                                           // [n_m + 1] (<= 65)
+    uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 2);                // [n_phi][RW][NT]
+    uint32_t *marg = hist + (size_t)n_phi * RW * NT;                                          // [n_phi][RW][NT]
+
+    const int lc = blockIdx.x / prm.jobs_per_lc;
+    const int job = blockIdx.x % prm.jobs_per_lc;
+    const int64_t tile_lo = prm.tiles_per_lc * job / prm.jobs_per_lc;
+    const int64_t tile_hi = prm.tiles_per_lc * (job + 1) / prm.jobs_per_lc;
+    const int n_tiles = (int)(tile_hi - tile_lo);
+    const int N = prm.info[lc].n;
+    const double dt_max = prm.info[lc].dt_max;
+    const double2 *gpts = prm.pts + prm.lc_offsets[lc];
+    const int n_chunks = (N + kChunk - 1) / kChunk;
+    const int total_seq = n_tiles * n_chunks;
+    const int64_t TILE = (int64_t)NT * R;
+
+    // ---- prologue: zero histograms, stage table / segments, start the TMA ring
+    for (int i = tid; i < n_phi * RW * NT * 2; i += NT) hist[i] = 0u;  // hist and marg are contiguous
+    for (int i = tid; i < kLtabSmem; i += NT) sL[i] = i < prm.ltab_n ? prm.ltab[i] : 0;
+    for (int i = tid; i <= n_m; i += NT) sseg[i] = prm.seg[(int64_t)lc * (n_m + 1) + i];
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); done[s] = 0; }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        for (int g = 0; g < kStages && g < total_seq; ++g) {
+            const int c = g % n_chunks;
+            const int cnt = min(kChunk, N - c * kChunk);
+            mbar_expect_tx(&full[g], (uint32_t)cnt * 16u);
+            tma_load_bulk(spts + g * kChunk, gpts + (size_t)c * kChunk, (uint32_t)cnt * 16u, &full[g]);
+        }
+    }
+    __syncthreads();
+
+    WarpTopK top;
+    top.reset(prm.top_k > 0 ? prm.top_k : 1);
+
+    const double nphi_d = (double)n_phi;
+    const double magic_b = kMagic + (double)prm.mod_bias;  // exact integer: floor(y) + bias in the low word
+    const uint32_t mod_mul = prm.mod_mul;
+    const uint32_t jstride = (uint32_t)(RW * NT) * 4u;     // bytes between consecutive phase bins
+    const uint32_t hbase = smem_u32(hist) + (uint32_t)tid * 4u;
+    const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)N : 0.0;
+
+    int g = 0;  // position in this CTA's chunk sequence
+    for (int tl = 0; tl < n_tiles; ++tl) {
+        const int64_t s0 = (tile_lo + tl) * TILE + (int64_t)tid * R;  // first trial slot of this thread
+        // ---- per-trial constants
+        double invP[R], cc[R];  // SHARE_P: only invP[0] is used
+        int64_t qv[R];
+        bool valid[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t s = s0 + r;
+            valid[r] = s < prm.n_trials;
+            int64_t q = 0;
+            if (valid[r]) q = DUMP ? prm.trial_q[s] : s;
+            qv[r] = q;
+            double ip = 0.0, c = 0.0;
+            if (valid[r]) trial_constants(prm.periods[q / prm.n_pdot], prm.pdots[q % prm.n_pdot], ip, c);
+            invP[r] = ip;
+            cc[r] = c;
+        }
+        // can this warp use the 32-bit floor/mod fast path for every point? (conservative bound on |y|)
+        bool fast = true;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double ip = invP[SHARE_P ? 0 : r];
+            const double yb = nphi_d * (dt_max * fabs(ip) + dt_max * dt_max * fabs(cc[r])) * 1.000001;
+            fast = fast && (yb < prm.y_safe);
+        }
+        fast = __all_sync(0xffffffffu, fast);
+
+        int64_t S2[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) S2[r] = 0;
+
+        int seg_i = 0;  // current magnitude bin
+        for (int c = 0; c < n_chunks; ++c, ++g) {
+            const int slot = g % kStages;
+            mbar_wait(&full[slot], (uint32_t)((g / kStages) & 1));
+            const double2 *sp = spts + slot * kChunk;
+            const int k_base = c * kChunk;
+            const int k_end = min(N, k_base + kChunk);
+            int k = k_base;
+            while (k < k_end) {
+                const int e = min(k_end, sseg[seg_i + 1]);
+                // ---------------- hot loop: fold + bin the points [k, e) of magnitude bin seg_i
+                if (fast) {
+                    // points are loaded in groups of kUnroll before any histogram update of the group, so the
+                    // broadcast LDS.128 of a group overlap (the updates are "memory"-clobbering asm)
+                    auto fold_bin_add = [&](const double2 p) {
+                        double a;
+                        if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
+                            const double b = __dmul_rn(p.y, cc[r]);
+                            const double x = __dadd_rn(a, b);
+                            const double y = __dmul_rn(x, nphi_d);
+                            const double z = __dadd_rd(y, magic_b);
+                            const uint32_t Iu = (uint32_t)__double2loint(z);      // floor(y) + bias >= 0
+                            const uint32_t qd = __umulhi(Iu, mod_mul);             // Iu / n_phi
+                            const uint32_t j = Iu - qd * (uint32_t)n_phi;          // Iu mod n_phi
+                            const uint32_t addr = hbase + j * jstride + (uint32_t)(r >> 1) * (uint32_t)NT * 4u;
+                            const uint32_t inc = (r & 1) ? 0x10000u : 1u;
+#if GCE_HIST_ATOMIC
+                            asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(inc) : "memory");
+#else
+                            uint32_t w;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(addr) : "memory");
+                            w += inc;
+                            asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(w) : "memory");
+#endif
+                        }
+                    };
+                    int kk = k - k_base;
+                    const int ke = e - k_base;
+                    for (; kk + kUnroll <= ke; kk += kUnroll) {
+                        double2 p[kUnroll];
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) p[u] = sp[kk + u];
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) fold_bin_add(p[u]);
+                    }
+                    for (; kk < ke; ++kk) fold_bin_add(sp[kk]);
+                } else {
+                    for (int kk = k - k_base; kk < e - k_base; ++kk) {
+                        const double2 p = sp[kk];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
+                            hist[((size_t)j * RW + (r >> 1)) * NT + tid] += (r & 1) ? 0x10000u : 1u;
+                        }
+                    }
+                }
+                k = e;
+                // ---------------- S4: close every magnitude bin that ends here (possibly several empty ones)
+                while (seg_i < n_m && sseg[seg_i + 1] == k) {
+                    for (int j = 0; j < n_phi; ++j) {
+#pragma unroll
+                        for (int w2 = 0; w2 < RW; ++w2) {
+                            const size_t idx = ((size_t)j * RW + w2) * NT + tid;
+                            const uint32_t w = hist[idx];
+                            if (w) {
+                                hist[idx] = 0u;
+                                marg[idx] += w;
+                            }
+                            const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
+                            S2[2 * w2] += c0 < kLtabSmem ? sL[c0] : prm.ltab[c0];
+                            if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += c1 < kLtabSmem ? sL[c1] : prm.ltab[c1];
+                            if (DUMP) {
+                                if (valid[2 * w2])
+                                    prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * n_m + seg_i] = c0;
+                                if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
+                                    prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * n_m + seg_i] = c1;
+                            }
+                        }
+                    }
+                    ++seg_i;
+                }
+            }
+            // ---------------- release the stage; the last warp to finish refills it (no dedicated producer)
+            __syncwarp();
+            if (lane == 0) {
+                __threadfence_block();
+                const int old = atomicAdd(&done[slot], 1);
+                if (old == NW - 1) {
+                    done[slot] = 0;
+                    const int gn = g + kStages;
+                    if (gn < total_seq) {
+                        const int cn = gn % n_chunks;
+                        const int cnt = min(kChunk, N - cn * kChunk);
+                        __threadfence_block();
+                        mbar_expect_tx(&full[slot], (uint32_t)cnt * 16u);
+                        tma_load_bulk(spts + slot * kChunk, gpts + (size_t)cn * kChunk, (uint32_t)cnt * 16u, &full[slot]);
+                    }
+                }
+            }
+        }
+        // trailing empty magnitude bins when N == 0 never occur (n_chunks == 0); DUMP tables stay zeroed by caller
+
+        // ---------------- finish the trials: S1 = sum_j L(n_j), CE, outputs
+        int64_t S1[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) S1[r] = 0;
+        if (N > 0) {
+            for (int j = 0; j < n_phi; ++j) {
+#pragma unroll
+                for (int w2 = 0; w2 < RW; ++w2) {
+                    const size_t idx = ((size_t)j * RW + w2) * NT + tid;
+                    const uint32_t w = marg[idx];
+                    marg[idx] = 0u;
+                    const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
+                    S1[2 * w2] += c0 < kLtabSmem ? sL[c0] : prm.ltab[c0];
+                    if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += c1 < kLtabSmem ? sL[c1] : prm.ltab[c1];
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t S = S1[r] - S2[r];  // = N * CE * 2^42, exact
+            const double ce = N > 0 ? (double)S * ce_scale : CUDART_NAN;
+            if (DUMP) {
+                if (valid[r] && prm.out_ce_at) prm.out_ce_at[(int64_t)lc * prm.n_trials + s0 + r] = ce;
+            } else {
+                if (valid[r] && prm.out_ce) {
+                    const int64_t o = (int64_t)lc * prm.n_trials + qv[r];
+                    if (prm.ce_fp64) reinterpret_cast<double *>(prm.out_ce)[o] = ce;
+                    else reinterpret_cast<float *>(prm.out_ce)[o] = (float)ce;
+                }
+                if (prm.top_k > 0) top.offer((valid[r] && N > 0) ? S : kInfS, (valid[r] && N > 0) ? qv[r] : kInfS);
+            }
+        }
+    }
+
+    // ---------------- per-CTA merge of the warps' top-k lists -> partial[lc][job][k]
+    if (!DUMP && prm.top_k > 0) {
+        const int K = prm.top_k;
+        __syncthreads();  // every issued TMA load has been consumed: the point ring is idle, reuse it as scratch
+        static_assert(sizeof(double2) * kStages * kChunk >= 16 * 32 * GCE_CE_MAX_TOPK, "scratch too small");
+        int64_t *scr = reinterpret_cast<int64_t *>(spts);
+        if (lane < K) {
+            scr[2 * ((tid >> 5) * K + lane)] = top.S;
+            scr[2 * ((tid >> 5) * K + lane) + 1] = top.q;
+        }
+        __syncthreads();
+        if (tid < 32) {
+            top.reset(K);
+            for (int e = 0; e < NW * K; e += 32) {
+                const int i = e + lane;
+                const int64_t cS = i < NW * K ? scr[2 * i] : kInfS;
+                const int64_t cq = i < NW * K ? scr[2 * i + 1] : kInfS;
+                top.offer(cS, cq);
+            }
+            if (lane < K) {
+                const int64_t o = ((int64_t)lc * prm.jobs_per_lc + job) * K + lane;
+                prm.part_S[o] = top.S;
+                prm.part_q[o] = top.q;
+            }
+        }
+    }
+}
+
+// One warp per light curve: merge jobs_per_lc x k candidates, write the user-facing selection.
+__global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ part_S, const int64_t *__restrict__ part_q,
+                                                   const LcInfo *__restrict__ info, int jobs_per_lc, int K,
+                                                   int64_t *__restrict__ out_idx, float *__restrict__ out_ce) {
+    const int lc = blockIdx.x, lane = threadIdx.x;
+    WarpTopK top;
+    top.reset(K);
+    const int total = jobs_per_lc * K;
+    for (int e = 0; e < total; e += 32) {
+        const int i = e + lane;
+        const int64_t cS = i < total ? part_S[(int64_t)lc * total + i] : kInfS;
+        const int64_t cq = i < total ? part_q[(int64_t)lc * total + i] : kInfS;
+        top.offer(cS, cq);
+    }
+    if (lane < K) {
+        const bool have = top.S != kInfS;
+        const int n = info[lc].n;
+        out_idx[(int64_t)lc * K + lane] = have ? top.q : -1;
+        if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)n)) : CUDART_NAN_F;
+    }
+}
+
+// Test-only: bins of one light curve for one trial, caller's point order (same device functions as the path).
+__global__ void k_debug_bins(const double *__restrict__ times, const double *__restrict__ mags,
+                             const int64_t *__restrict__ lc_offsets, const double *__restrict__ periods,
+                             const double *__restrict__ pdots, int64_t n_pdot, int n_phi, int n_m, int lc, int64_t q,
+                             uint32_t mod_mul, uint32_t mod_bias, double y_safe, int32_t *__restrict__ out_phase,
+                             int32_t *__restrict__ out_mag) {
+    __shared__ MinMax3 sh_red[8];
+    const int64_t off = lc_offsets[lc];
+    const int n = (int)(lc_offsets[lc + 1] - off);
+    const double *t = times + off, *m = mags + off;
+    MinMax3 v{CUDART_INF, -CUDART_INF, CUDART_INF, -CUDART_INF};
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const double tk = t[k], mk = m[k];
+        v.tmin = tk < v.tmin ? tk : v.tmin;
+        v.tmax = tk > v.tmax ? tk : v.tmax;
+        v.mmin = mk < v.mmin ? mk : v.mmin;
+        v.mmax = mk > v.mmax ? mk : v.mmax;
+    }
+    v = block_minmax(v, sh_red);
+    const double r = __dsub_rn(v.mmax, v.mmin);
+    double invP, c;
+    trial_constants(periods[q / n_pdot], pdots[q % n_pdot], invP, c);
+    const double dt_max = n > 0 ? __dsub_rn(v.tmax, v.tmin) : 0.0;
+    const bool fast = (double)n_phi * (dt_max * fabs(invP) + dt_max * dt_max * fabs(c)) * 1.000001 < y_safe;
+    const double magic_b = kMagic + (double)mod_bias;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const double dt = __dsub_rn(t[k], v.tmin), dt2 = __dmul_rn(dt, dt);
+        int j;
+        if (fast) {
+            const double y = __dmul_rn(__dadd_rn(__dmul_rn(dt, invP), __dmul_rn(dt2, c)), (double)n_phi);
+            const uint32_t Iu = (uint32_t)__double2loint(__dadd_rd(y, magic_b));
+            j = (int)(Iu - __umulhi(Iu, mod_mul) * (uint32_t)n_phi);
+        } else {
+            j = fold_bin_generic(dt, dt2, invP, c, n_phi);
+        }
+        out_phase[k] = j;
+        out_mag[k] = mag_bin(m[k], v.mmin, r, n_m);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+thread_local int g_last_cuda_error = 0;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t pts, seg, info, ltab, part_S, part_q, total;
+    int ltab_n;
+};
+
+struct Plan {
+    int R;
+    bool share_p;
+    int64_t tiles_per_lc;
+    int jobs_per_lc;
+};
+
+// Trials per thread and Pdot sharing: decided from sizes only (deterministic, no device query).
+Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int nt) {
+    Plan p;
+    p.R = 2;
+    p.share_p = (n_pdot % p.R) == 0;
+    const int64_t tile = (int64_t)nt * p.R;
+    p.tiles_per_lc = n_trials > 0 ? (n_trials + tile - 1) / tile : 0;
+    // ~16 CTAs per SM-slot overall for dynamic balance, at least one tile per job
+    int64_t want = (148LL * 16 + (n_lc > 0 ? n_lc : 1) - 1) / (n_lc > 0 ? n_lc : 1);
+    if (want < 1) want = 1;
+    if (want > p.tiles_per_lc) want = p.tiles_per_lc;
+    if (want < 1) want = 1;
+    if (want > 4096) want = 4096;
+    p.jobs_per_lc = (int)want;
+    return p;
+}
+
+constexpr int kPlanThreads = 512;  // threads per CTA assumed by the workspace plan (kernel may run fewer CTAs/SM)
+
+Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t n_pdot, const gce_ce_params *prm) {
+    Layout L;
+    size_t o = 0;
+    L.pts = o; o = align_up(o + sizeof(double2) * (size_t)(total_points > 0 ? total_points : 1), 256);
+    L.seg = o; o = align_up(o + sizeof(int32_t) * (size_t)(n_lc > 0 ? n_lc : 1) * (prm->n_mag_bins + 1), 256);
+    L.info = o; o = align_up(o + sizeof(LcInfo) * (size_t)(n_lc > 0 ? n_lc : 1), 256);
+    int64_t tn = total_points < GCE_CE_MAX_POINTS ? total_points : GCE_CE_MAX_POINTS;
+    L.ltab_n = (int)tn + 1;
+    L.ltab = o; o = align_up(o + sizeof(int64_t) * (size_t)L.ltab_n, 256);
+    const Plan p = make_plan(n_lc, n_trials, n_pdot, kPlanThreads);
+    const size_t parts = (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc * (size_t)(prm->top_k > 0 ? prm->top_k : 1);
+    L.part_S = o; o = align_up(o + sizeof(int64_t) * parts, 256);
+    L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
+    L.total = o;
+    return L;
+}
+
+int check_params(const gce_ce_params *prm) {
+    if (!prm) return GCE_CE_ERR_POINTER;
+    if (prm->n_phase_bins < 1 || prm->n_phase_bins > GCE_CE_MAX_BINS) return GCE_CE_ERR_RANGE;
+    if (prm->n_mag_bins < 1 || prm->n_mag_bins > GCE_CE_MAX_BINS) return GCE_CE_ERR_RANGE;
+    if (prm->top_k < 0 || prm->top_k > GCE_CE_MAX_TOPK) return GCE_CE_ERR_RANGE;
+    if (prm->ce_fp64 != 0 && prm->ce_fp64 != 1) return GCE_CE_ERR_RANGE;
+    if (prm->want_stats != 0 || prm->overlap != 0) return GCE_CE_ERR_RANGE;  // NEXT items N1 / N2: not yet built
+    if (prm->reserved[0] != 0 || prm->reserved[1] != 0) return GCE_CE_ERR_RANGE;
+    return GCE_CE_OK;
+}
+
+int check_sizes(int32_t n_lc, int64_t total_points, int64_t n_p, int64_t n_pdot) {
+    if (n_lc < 0 || total_points < 0 || n_p < 0 || n_pdot < 1) return GCE_CE_ERR_RANGE;
+    if (n_lc > (1 << 24)) return GCE_CE_ERR_RANGE;
+    if (n_p > 0 && n_pdot > (int64_t)0x7fffffffffffLL / n_p) return GCE_CE_ERR_RANGE;
+    return GCE_CE_OK;
+}
+
+// Exact 32-bit floor-mod constants: q = umulhi(I, M) equals I / d for I < nmax.
+void mod_constants(int d, uint32_t *mul, uint32_t *bias, double *y_safe) {
+    if (d == 1) { *mul = 0; *bias = 0; *y_safe = -1.0; return; }  // always the generic path (j = 0)
+    const uint64_t M = (1ULL << 32) / (uint64_t)d + 1;
+    const uint64_t e = M * (uint64_t)d - (1ULL << 32);
+    const uint64_t nmax = 0xffffffffULL / e;
+    const uint64_t half = nmax / 2;
+    const uint64_t B = half / (uint64_t)d * (uint64_t)d;
+    *mul = (uint32_t)M;
+    *bias = (uint32_t)B;
+    *y_safe = (double)(B - (uint64_t)d - 2);
+}
+
+int cuda_fail(cudaError_t e) {
+    g_last_cuda_error = (int)e;
+    return GCE_CE_ERR_CUDA;
+}
+
+size_t search_smem_bytes(int nt, int n_phi, int R) {
+    const int RW = (R + 1) / 2;
+    size_t fixed = sizeof(double2) * kStages * kChunk + sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * kStages +
+                   sizeof(int) * (kStages + 1) + sizeof(int) * (GCE_CE_MAX_BINS + 2);
+    return fixed + (size_t)2 * n_phi * RW * nt * sizeof(uint32_t);
+}
+
+template <int R, bool SHARE_P, bool DUMP>
+int launch_search(const SearchParams &sp, int32_t n_lc, cudaStream_t st) {
+    auto kern = k_search<R, SHARE_P, DUMP>;
+    // choose threads per CTA: the most resident threads per SM that registers and shared memory allow
+    int best_nt = 0, best_threads = 0;
+    const int cands[] = {1024, 768, 512, 384, 256, 128, 64, 32};
+    for (int nt : cands) {
+        const size_t smem = search_smem_bytes(nt, sp.n_phi, R);
+        if (smem > 227 * 1024) continue;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+            cudaGetLastError();
+            continue;
+        }
+        int blocks = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks, kern, nt, smem) != cudaSuccess) {
+            cudaGetLastError();
+            continue;
+        }
+        if (blocks * nt > best_threads) { best_threads = blocks * nt; best_nt = nt; }
+    }
+    if (best_nt == 0) return GCE_CE_ERR_RANGE;
+    // the workspace plan (partials) was sized for kPlanThreads; a smaller CTA would need more tiles per job, which
+    // is fine (jobs_per_lc is fixed by the plan), a larger one fewer.
+    SearchParams p = sp;
+    const int64_t tile = (int64_t)best_nt * R;
+    p.tiles_per_lc = p.n_trials > 0 ? (p.n_trials + tile - 1) / tile : 0;
+    if (p.jobs_per_lc > p.tiles_per_lc) {
+        // fewer tiles than planned jobs: surplus jobs get empty tile ranges (they still write +inf partials)
+    }
+    const size_t smem = search_smem_bytes(best_nt, p.n_phi, R);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail(e);
+    const unsigned grid = (unsigned)((int64_t)n_lc * p.jobs_per_lc);
+    kern<<<grid, best_nt, smem, st>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return GCE_CE_OK;
+}
+
+}  // namespace
+
+// ================================================================================================ C ABI
+extern "C" {
+
+const char *gce_ce_version(void) { return "gce-b200 0.1 (sm_100a)"; }
+
+const char *gce_ce_strerror(int code) {
+    switch (code) {
+        case GCE_CE_OK: return "ok";
+        case GCE_CE_ERR_POINTER: return "null or inconsistent pointer arguments";
+        case GCE_CE_ERR_RANGE: return "size, bin count or option out of range";
+        case GCE_CE_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case GCE_CE_ERR_CUDA: return "CUDA runtime error (see gce_ce_last_cuda_error)";
+        default: return "unknown error code";
+    }
+}
+
+int gce_ce_last_cuda_error(void) { return g_last_cuda_error; }
+
+int gce_ce_launch_count(int32_t n_lc, const gce_ce_params *prm) {
+    if (!prm || n_lc <= 0) return 0;
+    return 3 + (prm->top_k > 0 ? 1 : 0);  // preprocess, ltab, search, [merge]
+}
+
+int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int64_t n_pdot, const gce_ce_params *prm,
+                           size_t *bytes) {
+    if (!bytes) return GCE_CE_ERR_POINTER;
+    int rc = check_params(prm);
+    if (rc) return rc;
+    rc = check_sizes(n_lc, total_points, n_p, n_pdot);
+    if (rc) return rc;
+    *bytes = make_layout(total_points, n_lc, n_p * n_pdot, n_pdot, prm).total;
+    return GCE_CE_OK;
+}
+
+static int run_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                      int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                      const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                      const int64_t *trial_q, int64_t n_dump, uint32_t *out_counts, double *out_ce_at, void *workspace,
+                      size_t workspace_bytes, void *stream) {
+    const bool dump = out_counts != nullptr;
+    int rc = check_params(prm);
+    if (rc) return rc;
+    rc = check_sizes(n_lc, total_points, n_p, n_pdot);
+    if (rc) return rc;
+    if (!lc_offsets || !workspace) return GCE_CE_ERR_POINTER;
+    if (total_points > 0 && (!times || !mags)) return GCE_CE_ERR_POINTER;
+    if (n_p > 0 && !periods) return GCE_CE_ERR_POINTER;
+    if (!pdots) return GCE_CE_ERR_POINTER;
+    if (dump) {
+        if (!trial_q || n_dump < 0) return GCE_CE_ERR_POINTER;
+    } else {
+        if (!out_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+        if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
+        if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+    }
+    const int64_t n_trials = dump ? n_dump : n_p * n_pdot;
+    gce_ce_params lay_prm = *prm;
+    if (dump) lay_prm.top_k = 0;
+    const Layout L = make_layout(total_points, n_lc, n_trials, dump ? 1 : n_pdot, &lay_prm);
+    if (workspace_bytes < L.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return GCE_CE_ERR_WORKSPACE;
+    if (n_lc == 0) return GCE_CE_OK;
+
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    unsigned char *ws = reinterpret_cast<unsigned char *>(workspace);
+    double2 *pts = reinterpret_cast<double2 *>(ws + L.pts);
+    int32_t *seg = reinterpret_cast<int32_t *>(ws + L.seg);
+    LcInfo *info = reinterpret_cast<LcInfo *>(ws + L.info);
+    int64_t *ltab = reinterpret_cast<int64_t *>(ws + L.ltab);
+
+    k_preprocess<<<n_lc, 256, 0, st>>>(times, mags, lc_offsets, prm->n_mag_bins, pts, seg, info);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    k_ltab<<<(L.ltab_n + 255) / 256, 256, 0, st>>>(ltab, L.ltab_n);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+
+    const Plan plan = make_plan(n_lc, n_trials, dump ? 1 : n_pdot, kPlanThreads);
+    SearchParams sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.pts = pts; sp.seg = seg; sp.info = info; sp.lc_offsets = lc_offsets; sp.ltab = ltab;
+    sp.periods = periods; sp.pdots = pdots; sp.trial_q = trial_q;
+    sp.n_p = n_p; sp.n_pdot = n_pdot; sp.n_trials = n_trials;
+    sp.jobs_per_lc = plan.jobs_per_lc;
+    sp.n_phi = prm->n_phase_bins; sp.n_m = prm->n_mag_bins;
+    mod_constants(prm->n_phase_bins, &sp.mod_mul, &sp.mod_bias, &sp.y_safe);
+    sp.ltab_n = L.ltab_n;
+    sp.top_k = dump ? 0 : prm->top_k;
+    sp.ce_fp64 = prm->ce_fp64;
+    sp.out_ce = out_ce;
+    sp.part_S = reinterpret_cast<int64_t *>(ws + L.part_S);
+    sp.part_q = reinterpret_cast<int64_t *>(ws + L.part_q);
+    sp.out_counts = out_counts; sp.out_ce_at = out_ce_at;
+
+    if (n_trials > 0) {
+        if (dump) rc = launch_search<2, false, true>(sp, n_lc, st);
+        else if (plan.share_p) rc = launch_search<2, true, false>(sp, n_lc, st);
+        else rc = launch_search<2, false, false>(sp, n_lc, st);
+        if (rc) return rc;
+    }
+    if (!dump && prm->top_k > 0) {
+        k_merge_topk<<<n_lc, 32, 0, st>>>(sp.part_S, sp.part_q, info, n_trials > 0 ? plan.jobs_per_lc : 0, prm->top_k,
+                                          out_best_idx, out_best_ce);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return GCE_CE_OK;
+}
+
+int gce_ce_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                  int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                  const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce, double *out_stats,
+                  void *workspace, size_t workspace_bytes, void *stream) {
+    if (out_stats) return GCE_CE_ERR_RANGE;  // N1 not yet built
+    return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, out_ce,
+                      out_best_idx, out_best_ce, nullptr, 0, nullptr, nullptr, workspace, workspace_bytes, stream);
+}
+
+int gce_ce_debug_histogram(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                           int64_t total_points, const double *periods, int64_t n_p, const double *pdots,
+                           int64_t n_pdot, const gce_ce_params *prm, const int64_t *trial_q, int64_t n_trials,
+                           uint32_t *out_counts, double *out_ce_at, void *workspace, size_t workspace_bytes,
+                           void *stream) {
+    if (!out_counts) return GCE_CE_ERR_POINTER;
+    int rc = check_params(prm);
+    if (rc) return rc;
+    if (n_lc > 0 && n_trials > 0) {
+        cudaError_t e = cudaMemsetAsync(out_counts, 0,
+                                        sizeof(uint32_t) * (size_t)n_lc * (size_t)n_trials * prm->n_phase_bins * prm->n_mag_bins,
+                                        reinterpret_cast<cudaStream_t>(stream));
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, nullptr, nullptr,
+                      nullptr, trial_q, n_trials, out_counts, out_ce_at, workspace, workspace_bytes, stream);
+}
+
+int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                      const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot, const gce_ce_params *prm,
+                      int32_t lc, int64_t q, int32_t *out_phase_bin, int32_t *out_mag_bin, void *stream) {
+    int rc = check_params(prm);
+    if (rc) return rc;
+    if (!times || !mags || !lc_offsets || !periods || !pdots || !out_phase_bin || !out_mag_bin) return GCE_CE_ERR_POINTER;
+    if (n_pdot < 1 || n_p < 1 || lc < 0 || lc >= n_lc || q < 0 || q >= n_p * n_pdot) return GCE_CE_ERR_RANGE;
+    uint32_t mul, bias;
+    double y_safe;
+    mod_constants(prm->n_phase_bins, &mul, &bias, &y_safe);
+    k_debug_bins<<<1, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(times, mags, lc_offsets, periods, pdots, n_pdot,
+                                                                       prm->n_phase_bins, prm->n_mag_bins, lc, q, mul,
+                                                                       bias, y_safe, out_phase_bin, out_mag_bin);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return GCE_CE_OK;
+}
+
+int gce_ce_validate_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                         const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                         const gce_ce_params *prm) {
+    int rc = check_params(prm);
+    if (rc) return rc;
+    if (!lc_offsets) return GCE_CE_ERR_POINTER;
+    if (n_lc < 0 || n_p < 0 || n_pdot < 1) return GCE_CE_ERR_RANGE;
+    if (lc_offsets[0] != 0) return GCE_CE_ERR_RANGE;
+    for (int32_t l = 0; l < n_lc; ++l) {
+        const int64_t n = lc_offsets[l + 1] - lc_offsets[l];
+        if (n < 0 || n > GCE_CE_MAX_POINTS) return GCE_CE_ERR_RANGE;
+    }
+    const int64_t total = lc_offsets[n_lc];
+    if (total > 0 && (!times || !mags)) return GCE_CE_ERR_POINTER;
+    for (int64_t k = 0; k < total; ++k)
+        if (!(times[k] - times[k] == 0.0) || !(mags[k] - mags[k] == 0.0)) return GCE_CE_ERR_RANGE;  // NaN / inf
+    if (n_p > 0 && !periods) return GCE_CE_ERR_POINTER;
+    if (!pdots) return GCE_CE_ERR_POINTER;
+    for (int64_t i = 0; i < n_p; ++i)
+        if (!(periods[i] > 0.0) || !(periods[i] - periods[i] == 0.0)) return GCE_CE_ERR_RANGE;
+    for (int64_t i = 0; i < n_pdot; ++i)
+        if (!(pdots[i] - pdots[i] == 0.0)) return GCE_CE_ERR_RANGE;
+    return GCE_CE_OK;
+}
+
+int gce_ce_search_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                       const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                       const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                       double *out_stats) {
+    if (out_stats) return GCE_CE_ERR_RANGE;
+    int rc = check_params(prm);
+    if (rc) return rc;
+    if (!lc_offsets || n_lc < 0) return GCE_CE_ERR_POINTER;
+    const int64_t total = lc_offsets[n_lc];
+    rc = check_sizes(n_lc, total, n_p, n_pdot);
+    if (rc) return rc;
+    size_t ws_bytes = 0;
+    rc = gce_ce_workspace_bytes(total, n_lc, n_p, n_pdot, prm, &ws_bytes);
+    if (rc) return rc;
+    const size_t n_trials = (size_t)n_p * (size_t)n_pdot;
+    const size_t ce_bytes = out_ce ? (size_t)n_lc * n_trials * (prm->ce_fp64 ? 8 : 4) : 0;
+    const size_t k = (size_t)prm->top_k;
+
+    cudaStream_t st;
+    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return cuda_fail(e);
+    void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
+    void *d_ce = nullptr, *d_idx = nullptr, *d_bce = nullptr;
+    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocAsync(p, bytes ? bytes : 16, st); };
+    rc = GCE_CE_OK;
+    do {
+        if ((e = dalloc(&d_t, 8 * (size_t)total)) || (e = dalloc(&d_m, 8 * (size_t)total)) ||
+            (e = dalloc(&d_off, 8 * (size_t)(n_lc + 1))) || (e = dalloc(&d_p, 8 * (size_t)n_p)) ||
+            (e = dalloc(&d_pd, 8 * (size_t)n_pdot)) || (e = dalloc(&d_ws, ws_bytes)) ||
+            (e = dalloc(&d_ce, ce_bytes)) || (e = dalloc(&d_idx, 8 * (size_t)n_lc * k)) ||
+            (e = dalloc(&d_bce, 4 * (size_t)n_lc * k))) { rc = cuda_fail(e); break; }
+        if (total) {
+            cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
+            cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
+        }
+        cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st);
+        if (n_p) cudaMemcpyAsync(d_p, periods, 8 * (size_t)n_p, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st);
+        rc = gce_ce_search((const double *)d_t, (const double *)d_m, (const int64_t *)d_off, n_lc, total,
+                           (const double *)d_p, n_p, (const double *)d_pd, n_pdot, prm, out_ce ? d_ce : nullptr,
+                           out_best_idx ? (int64_t *)d_idx : nullptr, out_best_ce ? (float *)d_bce : nullptr, nullptr,
+                           d_ws, ws_bytes, st);
+        if (rc) break;
+        if (out_ce && ce_bytes) cudaMemcpyAsync(out_ce, d_ce, ce_bytes, cudaMemcpyDeviceToHost, st);
+        if (out_best_idx && k) cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
+        if (out_best_ce && k) cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
+    } while (0);
+    void *frees[] = {d_t, d_m, d_off, d_p, d_pd, d_ws, d_ce, d_idx, d_bce};
+    for (void *p : frees)
+        if (p) cudaFreeAsync(p, st);
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess && rc == GCE_CE_OK) rc = cuda_fail(e);
+    cudaStreamDestroy(st);
+    return rc;
+}
+
+}  // extern "C"

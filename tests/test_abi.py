@@ -1,0 +1,84 @@
+"""CPU-only checks of the boundary: the C-ABI library builds for sm_100a, loads, and exports every symbol
+include/gce_ce.h declares; host-side argument validation returns the documented codes (no kernel runs)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gce():
+    from paper_2006_06866_b200.build import build
+    build()
+    import paper_2006_06866_b200 as g
+    return g
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "gce_ce.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gce_ce_[a-z_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(gce):
+    from paper_2006_06866_b200.build import LIB
+    lib = C.CDLL(LIB)
+    syms = _declared_symbols()
+    assert len(syms) >= 10
+    for s in syms:
+        assert hasattr(lib, s), f"{s} declared in include/gce_ce.h but not exported"
+    assert set(syms) == set(gce.EXPORTS)
+    assert "sm_100a" in gce.gce_ce_version()
+
+
+def test_sass_is_sm100_and_uses_tma_bulk_copy(gce):
+    """The shipped cubin targets sm_100a and the search kernel stages points with TMA bulk copies (UBLKCP)."""
+    import subprocess
+    from paper_2006_06866_b200.build import LIB
+    out = subprocess.run(["cuobjdump", "-sass", LIB], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    assert "UBLKCP" in out
+    assert "DADD.RM" in out and "DMUL" in out     # fp64 fold with a round-down add (the exact floor)
+
+
+def test_workspace_and_error_codes_on_host(gce):
+    prm = gce.make_params(20, 10, top_k=5)
+    n = gce.gce_ce_workspace_bytes(64000, 64, 50000, 64, prm)
+    assert n > 64000 * 16 and n % 256 == 0
+    for bad in (gce.make_params(0, 10), gce.make_params(20, 65), gce.make_params(20, 10, top_k=33)):
+        with pytest.raises(gce.GceError) as e:
+            gce.gce_ce_workspace_bytes(100, 1, 10, 1, bad)
+        assert e.value.code == -2
+    with pytest.raises(gce.GceError):
+        gce.gce_ce_workspace_bytes(-1, 1, 10, 1, prm)
+    assert gce.gce_ce_launch_count(3, prm) == 4
+    assert gce.gce_ce_launch_count(3, gce.make_params(20, 10)) == 3
+
+
+def test_validate_host(gce):
+    prm = gce.make_params(20, 10)
+    t = np.arange(10.0)
+    m = np.sin(t)
+    assert gce.gce_ce_validate_host(t, m, [0, 4, 10], [100.0, 50.0], [0.0], prm) == 0
+    assert gce.gce_ce_validate_host(t, m, [0, 11, 10], [100.0], [0.0], prm) == -2      # non-monotone offsets
+    assert gce.gce_ce_validate_host(t, m, [0, 4, 10], [100.0, -1.0], [0.0], prm) == -2  # P <= 0
+    m2 = m.copy()
+    m2[3] = np.nan
+    assert gce.gce_ce_validate_host(t, m2, [0, 4, 10], [100.0], [0.0], prm) == -2
+
+
+def test_product_does_not_import_the_oracle():
+    """The product path must not route through the oracle (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2006_06866_b200")
+    for dirpath, _dirs, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "gce_oracle" not in src, f
+    opy = open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert not re.search(r"^\s*(import|from)\s+paper_2006_06866_b200", opy, flags=re.M)
+    assert "#include \"gce_ce" not in open(os.path.join(ROOT, "oracle", "gce_oracle.c")).read()

@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json:north_star): histogram counts and bin indices bit-exact; CE within 1e-5 relative (fp32
+output) or 1e-12 (fp64 output) and exactly 0 where the oracle's is exactly 0; best index equal to the
+oracle's except inside a near-tie class (|dCE| < rtol*CE), where the GPU's pick must lie in that class.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import gce_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+RTOL32, RTOL64 = 1e-5, 1e-12
+
+
+@pytest.fixture(scope="module")
+def gce():
+    from paper_2006_06866_b200.build import build
+    build()
+    import paper_2006_06866_b200 as g
+    return g
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_search(gce, w, top_k=None, want_cube=True, ce_fp64=False):
+    k = w.top_k if top_k is None else top_k
+    res = gce.search(dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots),
+                     w.n_phase_bins, w.n_mag_bins, top_k=k, want_cube=want_cube, ce_fp64=ce_fp64)
+    torch.cuda.synchronize()
+    return res
+
+
+def assert_ce_close(got, ref, rtol):
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    assert got.shape == ref.shape
+    nan = np.isnan(ref)
+    assert np.array_equal(np.isnan(got), nan)
+    g, r = got[~nan], ref[~nan]
+    assert np.all(g[r == 0.0] == 0.0), "CE must be exactly 0 where the oracle's is exactly 0"
+    # fixed-point table quantum (2^-43 per table entry, a few hundred entries) over N >= 1
+    err = np.abs(g - r)
+    bad = err > rtol * np.abs(r) + 1e-13
+    assert not bad.any(), f"max rel err {np.max(err / np.maximum(np.abs(r), 1e-300)):.3e} at {np.argmax(bad)}"
+
+
+def assert_topk_matches(ref_row, gpu_idx, gpu_val, k, rtol, oracle):
+    """Ordered-list comparison with the near-tie allowance at every rank and at the k / k+1 boundary."""
+    ref_row = np.asarray(ref_row, dtype=np.float64).ravel()
+    n_valid = int(np.sum(~np.isnan(ref_row)))
+    idx_ref, val_ref = oracle.topk(ref_row, min(k + 1, max(n_valid, 1)) if n_valid else k)
+    gpu_idx = np.asarray(gpu_idx)
+    assert gpu_idx.shape == (k,)
+    n_expect = min(k, n_valid)
+    assert np.all(gpu_idx[n_expect:] == -1)
+    assert np.all(np.isnan(np.asarray(gpu_val)[n_expect:]))
+    gi = gpu_idx[:n_expect]
+    assert len(set(gi.tolist())) == n_expect and np.all((gi >= 0) & (gi < ref_row.size))
+    for r in range(n_expect):
+        v_or = val_ref[r]
+        v_gpu_exact = ref_row[gi[r]]
+        # the trial the GPU put at rank r has (oracle) CE within the near-tie class of the oracle's rank-r CE
+        assert abs(v_gpu_exact - v_or) <= rtol * abs(v_or) + 1e-13, (r, gi[r], idx_ref[r], v_gpu_exact, v_or)
+        assert abs(float(gpu_val[r]) - v_gpu_exact) <= RTOL32 * abs(v_gpu_exact) + 1e-12
+        if gi[r] != idx_ref[r]:
+            # differing index is only allowed inside a near tie
+            assert abs(ref_row[idx_ref[r]] - v_gpu_exact) <= rtol * abs(v_or) + 1e-13
+
+
+# ------------------------------------------------------------------------------------------ bins (S1, S2)
+@pytest.mark.parametrize("n_phi,n_m", [(20, 10), (15, 8), (30, 10), (50, 10), (1, 1), (64, 64), (7, 3)])
+def test_debug_bins_bit_exact(gce, oracle, n_phi, n_m):
+    w = W.random_batch(100 + n_phi, n_lc=3, n_min=1, n_max=700, n_p=40, n_pdot=5, n_phase_bins=n_phi,
+                       n_mag_bins=n_m, pdot_range=(-2e-9, 3e-10))
+    prm = gce.make_params(n_phi, n_m)
+    t, m, o, p, pd = dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots)
+    for lc in range(w.n_lc):
+        a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
+        dt, dt2, mbin = oracle.preprocess(w.times[a:b], w.mags[a:b], n_m)
+        pb_gpu = torch.empty(b - a, dtype=torch.int32, device="cuda")
+        mb_gpu = torch.empty(b - a, dtype=torch.int32, device="cuda")
+        for q in (0, 7, 93, 199):
+            gce.gce_ce_debug_bins(t, m, o, p, pd, prm, lc, q, pb_gpu, mb_gpu)
+            pb, _ = oracle.fold_bins(dt, dt2, w.periods[q // 5], w.pdots[q % 5], n_phi)
+            assert np.array_equal(pb_gpu.cpu().numpy(), pb)
+            assert np.array_equal(mb_gpu.cpu().numpy(), mbin)
+
+
+def test_debug_bins_huge_cycle_counts_take_the_slow_path(gce, oracle):
+    """|n_phi * x| beyond the 32-bit fast range (and negative x for Pdot > 0) must still be bit-exact."""
+    rng = np.random.default_rng(3)
+    t = np.sort(rng.uniform(0, 3.0e9, size=300))
+    m = rng.normal(size=300)
+    periods = np.array([0.37, 1.0, 55.0, 420.0])
+    pdots = np.array([-1e-9, 0.0, 5e-8])
+    prm = gce.make_params(50, 10)
+    dt, dt2, mbin = oracle.preprocess(t, m, 10)
+    args = [dev(t), dev(m), dev(np.array([0, 300])), dev(periods), dev(pdots)]
+    pb_gpu = torch.empty(300, dtype=torch.int32, device="cuda")
+    mb_gpu = torch.empty(300, dtype=torch.int32, device="cuda")
+    for q in range(12):
+        gce.gce_ce_debug_bins(*args, prm, 0, q, pb_gpu, mb_gpu)
+        pb, x = oracle.fold_bins(dt, dt2, periods[q // 3], pdots[q % 3], 50)
+        assert np.array_equal(pb_gpu.cpu().numpy(), pb), q
+    assert x.min() < 0  # the Pdot > 0 trial really went negative
+
+
+# ------------------------------------------------------------------------------------------ counts (S3)
+@pytest.mark.parametrize("seed,n_phi,n_m,n_p,n_pdot", [(1, 20, 10, 37, 4), (2, 15, 8, 300, 1), (3, 30, 10, 64, 7),
+                                                        (4, 50, 10, 5, 3), (5, 1, 4, 9, 2), (6, 64, 64, 33, 2)])
+def test_histogram_counts_bit_exact(gce, oracle, seed, n_phi, n_m, n_p, n_pdot):
+    """Production search kernel in dump mode: counts identical to the oracle's for every sampled trial, on
+    ragged batches (incl. empty and 1-point light curves) longer than one shared-memory stage (512 points)."""
+    w = W.random_batch(seed, n_lc=5, n_min=0, n_max=1500, n_p=n_p, n_pdot=n_pdot, n_phase_bins=n_phi, n_mag_bins=n_m)
+    rng = np.random.default_rng(seed)
+    T = n_p * n_pdot
+    q = np.unique(np.concatenate([[0, T - 1], rng.integers(0, T, size=min(T, 70))])).astype(np.int64)
+    rng.shuffle(q)
+    prm = gce.make_params(n_phi, n_m)
+    ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, q.size, 1, prm), dtype=torch.uint8, device="cuda")
+    counts = torch.empty((w.n_lc, q.size, n_phi, n_m), dtype=torch.int32, device="cuda")
+    ce_at = torch.empty((w.n_lc, q.size), dtype=torch.float64, device="cuda")
+    gce.gce_ce_debug_histogram(dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots), prm,
+                               dev(q), counts, ce_at, ws)
+    torch.cuda.synchronize()
+    counts = counts.cpu().numpy()
+    ce_ref = oracle.ce_at(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, n_phi, n_m, q)
+    for lc in range(w.n_lc):
+        a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
+        ref = oracle.histogram(w.times[a:b], w.mags[a:b], w.periods, w.pdots, n_phi, n_m, q)
+        assert np.array_equal(counts[lc].astype(np.int64), ref), lc
+        assert np.all(counts[lc].sum(axis=(1, 2)) == b - a)
+    assert_ce_close(ce_at.cpu().numpy(), ce_ref, RTOL64)
+
+
+# ------------------------------------------------------------------------------------------ CE cube (S4) + selection (S5)
+def test_c1_full(gce, oracle):
+    """BASELINE.json:configs[0] at full size: full CE vector + argmin, fp32 and fp64 outputs."""
+    w = W.make("C1")
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 10)
+    for fp64, rtol in ((False, RTOL32), (True, RTOL64)):
+        res = run_search(gce, w, top_k=1, ce_fp64=fp64)
+        assert_ce_close(res.ce.cpu().numpy(), ref, rtol)
+        assert_topk_matches(ref[0], res.best_idx[0].cpu().numpy(), res.best_ce[0].cpu().numpy(), 1, rtol, oracle)
+    # the sinusoid's period (420 s) is recovered up to the grid step / a harmonic
+    P_best = w.periods[int(res.best_idx[0, 0])]
+    assert min(abs(P_best / 420.0 - h) for h in (0.5, 1.0, 2.0)) < 0.02
+
+
+@pytest.mark.parametrize("name,kw,k", [
+    ("C2", dict(n_lc=6, n_p=3000), 1),
+    ("C3", dict(n_lc=4, n_p=1500, n_pdot=64), 1),
+    ("C3", dict(n_lc=2, n_p=1111, n_pdot=7), 3),      # odd n_pdot: trials of a thread do not share a period
+    ("C4", dict(n_lc=9, n_p=5000), 5),
+    ("C5", dict(n_lc=2, n_p=300, n_pdot=16), 16),
+])
+def test_reduced_configs_cube_and_topk(gce, oracle, name, kw, k):
+    """The five workloads on reduced grids (same ranges): whole cube + fused top-k against the oracle."""
+    w = W.make(name, **kw)
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, w.n_phase_bins, w.n_mag_bins)
+    for fp64, rtol in ((False, RTOL32), (True, RTOL64)):
+        res = run_search(gce, w, top_k=k, ce_fp64=fp64)
+        assert_ce_close(res.ce.cpu().numpy(), ref, rtol)
+        for lc in range(w.n_lc):
+            assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), k, rtol, oracle)
+    # fused selection without a cube gives the same answer as with one
+    res2 = run_search(gce, w, top_k=k, want_cube=False)
+    assert torch.equal(res2.best_idx, res.best_idx)
+    # and equals a CPU reduction of the GPU's own fp64 cube, bit for bit (exact integer ordering inside)
+    cube64 = res.ce.cpu().numpy().reshape(w.n_lc, -1)
+    for lc in range(w.n_lc):
+        order = np.lexsort((np.arange(cube64.shape[1]), cube64[lc]))[:k]
+        assert np.array_equal(order, res.best_idx[lc].cpu().numpy())
+
+
+def test_ragged_batch_with_degenerate_light_curves(gce, oracle):
+    """Empty, 1-point, constant-magnitude and ordinary light curves in one batch; top_k larger than useful."""
+    rng = np.random.default_rng(8)
+    lcs = [
+        (np.zeros(0), np.zeros(0)),                                            # N = 0 -> NaN, idx -1
+        (np.array([5.0]), np.array([1.0])),                                    # N = 1 -> CE = 0
+        (np.sort(rng.uniform(0, 1e6, 333)), np.full(333, 17.0)),               # all magnitudes equal -> CE = 0
+        (rng.uniform(0, 1e7, 1029), rng.normal(size=1029)),                    # unsorted times
+        (np.sort(rng.uniform(0, 1e6, 64)), rng.normal(size=64)),
+    ]
+    times = np.concatenate([t for t, _ in lcs])
+    mags = np.concatenate([m for _, m in lcs])
+    offs = np.cumsum([0] + [t.size for t, _ in lcs]).astype(np.int64)
+    periods = 1.0 / np.linspace(1 / 5000.0, 1 / 50.0, 23)
+    pdots = np.linspace(-1e-9, 2e-10, 6)
+    ref = oracle.ce_search(times, mags, offs, periods, pdots, 20, 10)
+    w = W.Workload("ragged", times, mags, offs, periods, pdots, 20, 10, 32, True)
+    res = run_search(gce, w, top_k=32, ce_fp64=True)
+    got = res.ce.cpu().numpy()
+    assert_ce_close(got, ref, RTOL64)
+    assert np.all(np.isnan(got[0])) and np.all(got[1] == 0.0) and np.all(got[2] == 0.0)
+    assert np.all(res.best_idx[0].cpu().numpy() == -1)
+    assert np.array_equal(res.best_idx[1].cpu().numpy(), np.arange(32))       # all CE tie at 0 -> smallest q first
+    for lc in range(1, 5):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 32, RTOL64, oracle)
+
+
+def test_fewer_trials_than_k_and_single_trial(gce, oracle):
+    w = W.random_batch(12, n_lc=2, n_min=50, n_max=60, n_p=3, n_pdot=1)
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 10)
+    res = run_search(gce, w, top_k=8, ce_fp64=True)
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    for lc in range(2):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 8, RTOL64, oracle)
+
+
+def test_special_cases_on_gpu(gce, oracle):
+    """n_phi = 1 -> CE = H(m) for every trial; n_m = 1 -> CE = 0; bounds 0 <= CE <= ln n_m."""
+    w = W.random_batch(21, n_lc=2, n_min=200, n_max=400, n_p=50, n_pdot=2, n_phase_bins=1, n_mag_bins=10)
+    res = run_search(gce, w, top_k=0, ce_fp64=True)
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 1, 10)
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    assert np.ptp(res.ce[0].cpu().numpy()) == 0.0
+    w.n_phase_bins, w.n_mag_bins = 20, 1
+    assert torch.all(run_search(gce, w, top_k=0).ce == 0)
+    w.n_mag_bins = 10
+    ce = run_search(gce, w, top_k=0).ce
+    assert float(ce.min()) >= 0.0 and float(ce.max()) <= math.log(10) + 1e-6
+
+
+def test_host_entry_point_matches_device_entry_point(gce, oracle):
+    w = W.make("C3", n_lc=2, n_p=400, n_pdot=8)
+    prm = gce.make_params(20, 10, top_k=3)
+    ce = np.empty((2, 400, 8), dtype=np.float32)
+    idx = np.empty((2, 3), dtype=np.int64)
+    val = np.empty((2, 3), dtype=np.float32)
+    gce.gce_ce_search_host(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, prm, ce, idx, val)
+    res = run_search(gce, w, top_k=3)
+    assert np.array_equal(ce, res.ce.cpu().numpy())
+    assert np.array_equal(idx, res.best_idx.cpu().numpy())
+    assert np.array_equal(val, res.best_ce.cpu().numpy())
+
+
+def test_error_codes(gce):
+    w = W.make("C1", n_p=10)
+    t, m, o, p, pd = dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots)
+    prm = gce.make_params(20, 10, top_k=1)
+    ws = torch.empty(gce.gce_ce_workspace_bytes(200, 1, 10, 1, prm), dtype=torch.uint8, device="cuda")
+    ce = torch.empty(10, dtype=torch.float32, device="cuda")
+    idx = torch.empty(1, dtype=torch.int64, device="cuda")
+    with pytest.raises(gce.GceError) as e:      # top_k > 0 but no index output
+        gce.gce_ce_search(t, m, o, p, pd, prm, ce, None, None, None, ws)
+    assert e.value.code == -1
+    with pytest.raises(gce.GceError) as e:      # workspace too small
+        gce.gce_ce_search(t, m, o, p, pd, prm, ce, idx, None, None, ws[:256])
+    assert e.value.code == -3
+    with pytest.raises(gce.GceError) as e:      # bin count out of range
+        gce.gce_ce_workspace_bytes(200, 1, 10, 1, gce.make_params(65, 10))
+    assert e.value.code == -2
+    gce.gce_ce_search(t, m, o, p, pd, prm, ce, idx, None, None, ws)   # and the valid call goes through
+    torch.cuda.synchronize()
