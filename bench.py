@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- CE (P, Pdot) search throughput on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (S1..S5 of SURVEY.md section 8a: preprocess, fold + bin + entropy,
+cube store and/or fused top-k) over one batch of seeded synthetic light curves (gce_workloads, DESIGN.md
+section 5).  Default workload: C3 = BASELINE.json:configs[2], the paper's P-Pdot grid (64 light curves x
+1000 points x 50 000 periods x 64 Pdots, full fp32 CE cube + per-LC best): the configuration the
+north_star's roofline target is stated on and the largest one whose requested output includes the cube.
+
+metric  : CE point-folds per second = n_lc * n_p * n_pdot * N_obs / t   (BASELINE.json:metric)
+value   : inputs already resident in HBM, CUDA-event time of the gce_ce_search enqueue, L2 flushed between steps
+e2e     : the same through gce_ce_search_host with pinned HOST buffers (H2D of the inputs, D2H of the outputs
+          and device allocation inside the timed region)
+roofline: the fold+bin+entropy kernel (k_search) against the FP64-pipe issue roofline,
+          timed live with CUDA events recorded by the library around that kernel
+cpu_baseline: the oracle (oracle/, as it stands) on this box's host cores over a bounded sample of the workload
+
+N > 1 (torchrun, one process per GPU): light curves are independent, so each rank searches its own batch of
+the same shape (seed offset by rank; weak scaling, no data-path collective); value = all ranks' point-folds /
+max-over-ranks time.  --impl reference times the oracle instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gce_workloads as W  # noqa: E402
+
+METRIC = "CE point-folds/sec"
+UNIT = "point-folds/s"
+FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (probe-measured)
+N_SM = 148
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.thr, self.index = [], None, None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append((time.time(), line.strip()))
+        self.thr = threading.Thread(target=pump, daemon=True)
+        self.thr.start()
+
+    def stop(self, t0=None, t1=None):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if (t0 is None or t >= t0) and (t1 is None or t <= t1 + 0.1)] or \
+               [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(name, rank, shrink):
+    kw = {}
+    if shrink:  # --quick: same ranges, smaller grid (for smoke-testing the bench itself; never a reported number)
+        kw = {"C1": {}, "C2": dict(n_lc=8, n_p=2000), "C3": dict(n_lc=4, n_p=2000, n_pdot=64),
+              "C4": dict(n_lc=16, n_p=4000), "C5": dict(n_lc=2, n_p=512, n_pdot=32)}[name]
+    if rank > 0:
+        # weak scaling: every rank owns a batch of the same shape; rank r re-draws it from seed + 1000 r
+        kw = dict(kw, seed={"C1": 0, "C2": 1, "C3": 2, "C4": 3, "C5": 4}[name] + 1000 * rank)
+    return W.make(name, **kw)
+
+
+def algorithmic_fp64_ops_per_pointfold(w):
+    """DMUL a=dt*invP (shared by the Pdot values of one period), DMUL b=dt2*c, DADD x=a+b,
+    DMUL y=x*n_phi, DADD.RD floor  ->  4 + 1/n_pdot per point-fold; 3 when the grid is Pdot = {0} only."""
+    if w.n_pdot == 1 and float(w.pdots[0]) == 0.0:
+        return 3.0
+    return 4.0 + 1.0 / w.n_pdot
+
+
+# ----------------------------------------------------------------------------------------- reference arm
+def oracle_sample(w, seconds_target):
+    """Bounded sample of the workload for the oracle: all light curves, all Pdots, a strided subset of the
+    periods sized from a short calibration run so one pass takes about `seconds_target` seconds."""
+    import oracle
+    oracle.build()
+    n_cal = max(1, min(w.n_p, int(2e8 // max(1, w.total_points * w.n_pdot))))
+    cal = w.subset(p_idx=np.linspace(0, w.n_p - 1, n_cal).astype(np.int64))
+    t = time.perf_counter()
+    oracle.ce_search(cal.times, cal.mags, cal.lc_offsets, cal.periods, cal.pdots, w.n_phase_bins, w.n_mag_bins)
+    dt = max(time.perf_counter() - t, 1e-4)
+    rate = cal.point_folds / dt
+    n_s = int(min(w.n_p, max(n_cal, rate * seconds_target // max(1, w.total_points * w.n_pdot))))
+    idx = np.unique(np.linspace(0, w.n_p - 1, n_s).astype(np.int64))
+    return w.subset(p_idx=idx), f"all {w.n_lc} light curves x {idx.size} of {w.n_p} periods (uniform stride) x all {w.n_pdot} Pdots"
+
+
+def time_oracle(sample, w):
+    import oracle
+    t = time.perf_counter()
+    oracle.ce_search(sample.times, sample.mags, sample.lc_offsets, sample.periods, sample.pdots,
+                     w.n_phase_bins, w.n_mag_bins)
+    return time.perf_counter() - t
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    w = make_workload(args.config, 0, args.quick)
+    per_step = max(1.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    sample, desc = oracle_sample(w, per_step)
+    for _ in range(args.warmup):
+        time_oracle(sample, w)
+    ts = [time_oracle(sample, w) for _ in range(args.steps)]
+    tot = float(sum(ts))
+    val = sample.point_folds * args.steps / tot
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, args),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(w, args):
+    return {"workload": f"{w.name} (BASELINE.json:configs[{int(w.name[1]) - 1}])" + (" QUICK-SHRUNK" if args.quick else ""),
+            "n_lc": w.n_lc, "n_obs_total": w.total_points, "n_p": w.n_p, "n_pdot": w.n_pdot,
+            "n_phase_bins": w.n_phase_bins, "n_mag_bins": w.n_mag_bins, "top_k": w.top_k, "ce_cube": bool(w.want_cube),
+            "point_folds_per_step_per_gpu": w.point_folds, "parallelism": f"independent light-curve batches x{args.gpus}",
+            "l2": "flushed between timed steps (256 MiB write), each step timed by its own CUDA-event pair"}
+
+
+# ----------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2006_06866_b200.build import build
+    if rank == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+    import paper_2006_06866_b200 as gce
+
+    w = make_workload(args.config, rank, args.quick)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    times, mags, offs, periods, pdots = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
+    k = w.top_k
+    ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev_a.record(); ev_b.record()  # forces creation of the cudaEvent_t handles
+    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k, ev_search_begin=ev_a, ev_search_end=ev_b)
+    ce = torch.empty((w.n_lc, w.n_p, w.n_pdot), dtype=torch.float32, device=dev) if w.want_cube else None
+    bidx = torch.empty((w.n_lc, k), dtype=torch.int64, device=dev) if k else None
+    bce = torch.empty((w.n_lc, k), dtype=torch.float32, device=dev) if k else None
+    ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, w.n_p, w.n_pdot, prm), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    launches_per_step = gce.gce_ce_launch_count(w.n_lc, prm)
+
+    def step():
+        gce.gce_ce_search(times, mags, offs, periods, pdots, prm, ce, bidx, bce, None, ws)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sync_all()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    s_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    e_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    k_ms = []
+    sync_all()
+    t_wall0 = time.time()
+    for i in range(args.steps):
+        flush.zero_()                       # evict L2 (126 MB) between timed steps; not inside the event pair
+        s_ev[i].record()
+        step()
+        e_ev[i].record()
+        e_ev[i].synchronize()               # the library's kernel-only events are reused every step
+        k_ms.append(ev_a.elapsed_time(ev_b))
+    sync_all()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    step_ms = [s.elapsed_time(e) for s, e in zip(s_ev, e_ev)]
+    tot_ms = float(sum(step_ms))
+    t = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
+    pf = torch.tensor([float(w.point_folds)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(pf, op=dist.ReduceOp.SUM)
+    tot_ms_max, pf_all = float(t.item()), float(pf.item())
+    value = pf_all * args.steps / (tot_ms_max * 1e-3)
+
+    # ---- end to end through the host entry point: pinned host buffers, H2D + D2H + allocation inside the timing
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_in = [pin(w.times), pin(w.mags), pin(w.lc_offsets), pin(w.periods), pin(w.pdots)]
+    h_ce = torch.empty((w.n_lc, w.n_p, w.n_pdot), dtype=torch.float32).pin_memory() if w.want_cube else None
+    h_idx = torch.empty((w.n_lc, k), dtype=torch.int64).pin_memory() if k else None
+    h_bce = torch.empty((w.n_lc, k), dtype=torch.float32).pin_memory() if k else None
+    prm_h = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k)
+    h2d = sum(x.numel() * x.element_size() for x in h_in)
+    d2h = sum(x.numel() * x.element_size() for x in (h_ce, h_idx, h_bce) if x is not None)
+    n_e2e = max(1, min(args.steps, 5))
+    gce.gce_ce_search_host(*h_in, prm_h, h_ce, h_idx, h_bce)   # warm-up (allocator pools)
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        gce.gce_ce_search_host(*h_in, prm_h, h_ce, h_idx, h_bce)  # synchronises before returning
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = pf_all * n_e2e / float(te.item())
+    if k and rank == 0:
+        assert torch.equal(h_idx.to(dev), bidx), "host and device entry points disagree"
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (k_search): FP64 pipe issue rate
+    peaks, peaks_src = load_peaks()
+    k_ms_avg = float(np.mean(k_ms))
+    ops = algorithmic_fp64_ops_per_pointfold(w) * w.point_folds
+    achieved = ops / (k_ms_avg * 1e-3) / 1e9                      # G lane-ops / s
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak = FP64_LANES_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9      # at the maximum SM clock (strictest denominator)
+    roof = {"bound": "alu", "pipe": "fp64", "kernel": "k_search", "achieved": achieved, "peak": peak,
+            "unit": "G FP64 lane-ops/s", "frac": achieved / peak, "traffic": None,
+            "peak_source": f"64 FP64 lanes/SM/clk x 148 SMs x {sm_max:.0f} MHz (max SM clock, {peaks_src} MEASURED_PEAKS.json; "
+                           "per-SM rate probe-measured, DESIGN.md section 7)",
+            "algorithmic_ops_per_point_fold": algorithmic_fp64_ops_per_pointfold(w),
+            "kernel_ms": k_ms_avg, "kernel_share_of_step": k_ms_avg * args.steps / tot_ms,
+            "frac_at_observed_clock": (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks and clocks.get("sm_mhz") else None,
+            "ce_output_gbs": (w.n_lc * w.n_p * w.n_pdot * 4 / (k_ms_avg * 1e-3) / 1e9) if w.want_cube else 0.0,
+            "hbm_peak_gbs": peaks.get("hbm_gbs")}
+
+    # ---- the oracle on this box's host cores, bounded sample
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        sample, desc = oracle_sample(w, 15.0)
+        t_cpu = time_oracle(sample, w)
+        cpu = {"value": sample.point_folds / t_cpu, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": desc, "seconds": t_cpu}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(w, args),
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
+                    "api": "gce_ce_search_host (pinned host buffers; cudaMallocAsync + H2D + search + D2H + sync)"},
+            "gpu_launches": launches_per_step * args.steps, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--quick", action="store_true", help="shrunk grid, to test the bench itself; not a reportable number")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -159,9 +159,9 @@ def _freq_grid(f_lo, f_hi, n):
 
 
 # ----------------------------------------------------------------------------- the five configs
-def config_c1(n_p=1000) -> Workload:
+def config_c1(n_p=1000, seed=0) -> Workload:
     """BASELINE.json:configs[0] -- one sinusoid, 200 points over 30 days, 1000 frequencies."""
-    rng = np.random.default_rng(0)
+    rng = np.random.default_rng(seed)
     t = np.sort(rng.uniform(0.0, 30.0 * DAY, size=200))
     mag = 0.2 * np.sin(2.0 * np.pi * t / 420.0) + rng.normal(0.0, 0.05, size=200)
     t = t - t[0]
@@ -185,18 +185,18 @@ def _two_dip_batch(seed, n_lc, cadence, p_lo, p_hi, pdot_log10, d1_rng, d2_rng, 
     return lcs, {"P": np.asarray(Ps), "Pdot": np.asarray(Pds)}
 
 
-def config_c2(n_lc=100, n_p=10_000) -> Workload:
+def config_c2(n_lc=100, n_p=10_000, seed=1) -> Workload:
     """BASELINE.json:configs[1] -- 100 ZTF-like LCs (N=500, 2 yr), 1e4 frequencies, Pdot={0}."""
-    lcs, truth = _two_dip_batch(1, n_lc, lambda r: ztf_like_cadence(r, 2, 500), 300.0, 3600.0, None,
+    lcs, truth = _two_dip_batch(seed, n_lc, lambda r: ztf_like_cadence(r, 2, 500), 300.0, 3600.0, None,
                                 (0.1, 0.8), (0.05, 0.4), 0.03)
     times, mags, offs = _pack(lcs)
     return Workload("C2", times, mags, offs, _freq_grid(1 / 7200.0, 1 / 180.0, n_p), np.zeros(1),
                     20, 10, top_k=1, want_cube=False, truth=truth)
 
 
-def config_c3(n_lc=64, n_p=50_000, n_pdot=64) -> Workload:
+def config_c3(n_lc=64, n_p=50_000, n_pdot=64, seed=2) -> Workload:
     """BASELINE.json:configs[2] -- the P-Pdot grid: 64 LCs (N=1000, 3 yr) x 5e4 freqs x 64 Pdots."""
-    lcs, truth = _two_dip_batch(2, n_lc, lambda r: ztf_like_cadence(r, 3, 1000), 180.0, 900.0, (-12.0, -10.0),
+    lcs, truth = _two_dip_batch(seed, n_lc, lambda r: ztf_like_cadence(r, 3, 1000), 180.0, 900.0, (-12.0, -10.0),
                                 (0.1, 0.8), (0.05, 0.4), 0.05)
     times, mags, offs = _pack(lcs)
     return Workload("C3", times, mags, offs, _freq_grid(1 / 1200.0, 1 / 120.0, n_p),
@@ -204,18 +204,18 @@ def config_c3(n_lc=64, n_p=50_000, n_pdot=64) -> Workload:
                     20, 10, top_k=1, want_cube=True, truth=truth)
 
 
-def config_c4(n_lc=1000, n_p=100_000) -> Workload:
+def config_c4(n_lc=1000, n_p=100_000, seed=3) -> Workload:
     """BASELINE.json:configs[3] -- LSST-like sparse batch: 1000 LCs (N=200, 10 yr), 1e5 freqs, top-5."""
-    lcs, truth = _two_dip_batch(3, n_lc, lambda r: lsst_like_cadence(r, 200), 600.0, 7200.0, None,
+    lcs, truth = _two_dip_batch(seed, n_lc, lambda r: lsst_like_cadence(r, 200), 600.0, 7200.0, None,
                                 (0.05, 0.5), (0.05, 0.5), 0.08)
     times, mags, offs = _pack(lcs)
     return Workload("C4", times, mags, offs, _freq_grid(1 / 14400.0, 1 / 300.0, n_p), np.zeros(1),
                     15, 8, top_k=5, want_cube=False, truth=truth)
 
 
-def config_c5(n_lc=16, n_p=1 << 17, n_pdot=256) -> Workload:
+def config_c5(n_lc=16, n_p=1 << 17, n_pdot=256, seed=4) -> Workload:
     """BASELINE.json:configs[4] -- heavy high-cadence P-Pdot search: 16 LCs (N=5000), 2^17 x 256, top-16."""
-    lcs, truth = _two_dip_batch(4, n_lc, lambda r: high_cadence_blocks(r), 120.0, 600.0, (-11.0, -9.0),
+    lcs, truth = _two_dip_batch(seed, n_lc, lambda r: high_cadence_blocks(r), 120.0, 600.0, (-11.0, -9.0),
                                 (0.1, 0.8), (0.05, 0.4), 0.02)
     times, mags, offs = _pack(lcs)
     return Workload("C5", times, mags, offs, _freq_grid(1 / 900.0, 1 / 90.0, n_p),
@@ -227,7 +227,8 @@ CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "
 
 
 def make(name: str, **kw) -> Workload:
-    """make("C3") -> full-size workload; keyword overrides shrink n_lc / n_p / n_pdot (same ranges)."""
+    """make("C3") -> full-size workload; keyword overrides shrink n_lc / n_p / n_pdot (same ranges); `seed`
+    overrides the configuration's own seed (used for the other ranks' batches in weak-scaling runs)."""
     return CONFIGS[name.upper()](**kw)
 
 

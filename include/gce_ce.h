@@ -55,6 +55,10 @@ typedef struct gce_ce_params {
     int32_t want_stats;   /* 1: out_stats receives the Eq. 5 statistics (requires out_stats)      */
     int32_t overlap;      /* 0: plain bins (hot path).  1: 50 % overlapping phase bins (:106, N2)  */
     int32_t reserved[2];  /* must be 0                                                            */
+    /* Optional cudaEvent_t handles (NULL = none), recorded on `stream` immediately before / after the
+     * fold+bin+entropy kernel, so a harness can time the dominant kernel alone without a profiler.    */
+    void *ev_search_begin;
+    void *ev_search_end;
 } gce_ce_params;
 
 /* Bytes of device workspace gce_ce_search needs for these sizes (256-byte aligned base required).

@@ -11,7 +11,7 @@ import importlib
 _BINDING_NAMES = (
     "EXPORTS", "GceError", "Params", "SearchResult", "gce_ce_debug_bins", "gce_ce_debug_histogram",
     "gce_ce_launch_count", "gce_ce_search", "gce_ce_search_host", "gce_ce_validate_host", "gce_ce_version",
-    "gce_ce_workspace_bytes", "gce_ce_last_cuda_error", "gce_ce_strerror", "make_params", "search", "SearchPlan",
+    "gce_ce_workspace_bytes", "make_params", "search",
 )
 
 

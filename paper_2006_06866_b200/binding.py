@@ -27,7 +27,7 @@ OK, ERR_POINTER, ERR_RANGE, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
 class Params(C.Structure):
     _fields_ = [("n_phase_bins", C.c_int32), ("n_mag_bins", C.c_int32), ("top_k", C.c_int32),
                 ("ce_fp64", C.c_int32), ("want_stats", C.c_int32), ("overlap", C.c_int32),
-                ("reserved", C.c_int32 * 2)]
+                ("reserved", C.c_int32 * 2), ("ev_search_begin", C.c_void_p), ("ev_search_end", C.c_void_p)]
 
 
 _vp, _i32, _i64, _sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
@@ -71,9 +71,14 @@ def gce_ce_version() -> str:
     return _lib.gce_ce_version().decode()
 
 
-def make_params(n_phase_bins, n_mag_bins, top_k=0, ce_fp64=False, want_stats=False, overlap=False) -> Params:
+def make_params(n_phase_bins, n_mag_bins, top_k=0, ce_fp64=False, want_stats=False, overlap=False,
+                ev_search_begin=None, ev_search_end=None) -> Params:
+    """ev_search_begin / ev_search_end: optional torch.cuda.Event(enable_timing=True) objects that have been
+    recorded at least once (torch creates the cudaEvent_t lazily); the caller keeps them alive."""
+    def _ev(e):
+        return None if e is None else C.c_void_p(e.cuda_event)
     return Params(int(n_phase_bins), int(n_mag_bins), int(top_k), int(bool(ce_fp64)), int(bool(want_stats)),
-                  int(bool(overlap)), (C.c_int32 * 2)(0, 0))
+                  int(bool(overlap)), (C.c_int32 * 2)(0, 0), _ev(ev_search_begin), _ev(ev_search_end))
 
 
 def gce_ce_workspace_bytes(total_points, n_lc, n_p, n_pdot, prm: Params) -> int:

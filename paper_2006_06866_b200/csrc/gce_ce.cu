@@ -800,11 +800,19 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.part_q = reinterpret_cast<int64_t *>(ws + L.part_q);
     sp.out_counts = out_counts; sp.out_ce_at = out_ce_at;
 
+    if (prm->ev_search_begin) {
+        e = cudaEventRecord(reinterpret_cast<cudaEvent_t>(prm->ev_search_begin), st);
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
     if (n_trials > 0) {
         if (dump) rc = launch_search<2, false, true>(sp, n_lc, st);
         else if (plan.share_p) rc = launch_search<2, true, false>(sp, n_lc, st);
         else rc = launch_search<2, false, false>(sp, n_lc, st);
         if (rc) return rc;
+    }
+    if (prm->ev_search_end) {
+        e = cudaEventRecord(reinterpret_cast<cudaEvent_t>(prm->ev_search_end), st);
+        if (e != cudaSuccess) return cuda_fail(e);
     }
     if (!dump && prm->top_k > 0) {
         k_merge_topk<<<n_lc, 32, 0, st>>>(sp.part_S, sp.part_q, info, n_trials > 0 ? plan.jobs_per_lc : 0, prm->top_k,
