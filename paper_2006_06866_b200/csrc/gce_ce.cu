@@ -10,12 +10,17 @@
 //   k_merge_topk  S5  per-light-curve merge of the per-CTA candidates
 //
 // Design (B200-first): one THREAD owns R consecutive trials (the paper's one-thread-
-// per-grid-point idea, :152, kept because it makes every shared-memory access conflict-free), the light curve
-// is streamed through a small ring of shared-memory stages by TMA bulk copies (cp.async.bulk + mbarrier) and
-// is shared by every thread of the CTA (broadcast LDS.128), points are pre-grouped by magnitude bin so a trial
-// only needs a 1-D phase histogram at a time (the paper's memory insight, :152), counters are 16-bit pairs in
-// a [bin][thread] column layout (bank = lane), and the entropy is accumulated in 2^-42 fixed point so CE does
-// not depend on summation order.  No tensor cores: this is a histogram/entropy path, not a contraction.
+// per-grid-point idea, :152, kept because it makes every shared-memory access conflict-free).  The R trials of a
+// thread share one period whenever n_pdot % R == 0, so a = dt * invP is computed once per point.  The whole light
+// curve is staged in shared memory by TMA bulk copies (cp.async.bulk + mbarrier) once per CTA and read by every
+// thread as a broadcast LDS.128; light curves longer than the buffer are streamed through two half buffers.
+// Points are pre-grouped by magnitude bin so a trial only needs a 1-D phase histogram at a time (the paper's
+// memory insight, :152); counters are 16-bit pairs in a [bin][thread] column layout (bank = lane), updated with
+// one RED.shared per point-fold; the phase marginal lives in registers (compile-time n_phi) and the entropy is
+// accumulated in 2^-42 fixed point so CE does not depend on summation order.  The phase bin is
+// floor(y) - n_phi * floor(x) from two round-down magic adds (exact for |y| < 2^51, no integer division: on sm_100
+// IMAD.HI is quarter rate and slows the FP64 pipe, measured in DESIGN.md section 7).  No tensor cores: this is a
+// histogram/entropy path, not a contraction.
 //
 // This translation unit must be compiled with -fmad=false; the fold additionally uses explicit _rn/_rd
 // intrinsics, which are never contracted.
@@ -32,13 +37,13 @@
 
 namespace {
 
-constexpr int kChunk = 512;       // points per shared-memory stage (16 B each -> 8 KB)
-constexpr int kStages = 3;        // TMA ring depth
-constexpr int kUnroll = 2;        // points loaded ahead per thread in the hot loop
 constexpr int kLtabSmem = 1024;   // entries of the L table mirrored in shared memory
 constexpr int kLfixShift = 42;    // L table fixed point: 2^-42
 constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(y) in the low mantissa word
+constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
 constexpr int64_t kInfS = INT64_MAX;
+constexpr int kSmemLimit = 227 * 1024;
+constexpr int kFastLog2NT = 9;    // the compile-time-n_phi kernels run 512 threads per CTA
 
 struct LcInfo {
     int32_t n;
@@ -59,8 +64,8 @@ struct SearchParams {
     int64_t tiles_per_lc;
     int32_t jobs_per_lc;
     int32_t n_phi, n_m;
-    uint32_t mod_mul, mod_bias;
-    double y_safe;             // |y| below this -> 32-bit fast floor/mod path is exact
+    int32_t log2nt;            // threads per CTA = 1 << log2nt
+    int32_t cap_points;        // capacity of the shared-memory point buffer (multiple of 8)
     int32_t ltab_n;
     int32_t top_k;
     int32_t ce_fp64;
@@ -249,25 +254,130 @@ __global__ void k_ltab(int64_t *__restrict__ ltab, int n) {
 }
 
 // ------------------------------------------------------------------------------------------------ S2..S5
-// R = trials per thread (1, 2 or 4).  SHARE_P: the R trials of a thread share one period (n_pdot % R == 0), so
-// a = dt * invP is computed once (bit-identical: a does not depend on Pdot).  DUMP: test mode, trials come from
-// a list and the count tables are written out.
-template <int R, bool SHARE_P, bool DUMP>
-__global__ void __launch_bounds__(1024, 1) k_search(const SearchParams prm) {
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+    uint32_t w;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(addr) : "memory");
+    return w;
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t w) {
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(w) : "memory");
+}
+__device__ __forceinline__ void red_add_u32(uint32_t addr, uint32_t inc) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(inc) : "memory");
+}
+
+// L(k) = k ln k in 2^-42 fixed point: first kLtabSmem entries from shared memory, the (rare) rest from global.
+__device__ __forceinline__ int64_t ltab_at(const int64_t *__restrict__ sL, const int64_t *__restrict__ gL, uint32_t c) {
+    int64_t v = sL[c & (kLtabSmem - 1)];
+    if (c >= (uint32_t)kLtabSmem) v = gL[c];
+    return v;
+}
+
+// S2 + S3 for one point and the R trials of this thread (DESIGN.md section 3; PAPER.md:100 Eq. 3, :106).
+//   a = dt*invP ; b = dt2*c ; x = a + b ; y = x*n_phi          (RN each, never fused)
+//   j = floor(y) - n_phi*floor(x)                               two exact round-down magic adds, |y| < 2^51
+// j equals floor(y) mod n_phi except when RN(x*n_phi) lands exactly on the next multiple of n_phi, where it is
+// n_phi: that count goes to an extra histogram row that is folded into row 0 when the segment is closed.
+// PZ: every trial of the thread has c = +-0, so x = a bit for bit (a >= +0) and two operations are skipped.
+template <int R, bool SHARE_P, bool PZ>
+__device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
+                                             const double nphi_d, const uint32_t negn, const uint32_t ls,
+                                             const uint32_t (&hb)[(R + 1) / 2]) {
+    double a;
+    if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
+        const double x = PZ ? a : __dadd_rn(a, __dmul_rn(p.y, cc[r]));
+        const double y = __dmul_rn(x, nphi_d);
+        const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
+        const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
+        const uint32_t j = Iy + Ix * negn;
+        red_add_u32((j << ls) + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
+    }
+}
+
+// Hot loop over the points [kk, ke) of one shared-memory buffer (all of one magnitude bin).
+template <int R, bool SHARE_P, bool PZ>
+__device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
+                                           const double (&cc)[R], const double nphi_d, const uint32_t negn,
+                                           const uint32_t ls, const uint32_t (&hb)[(R + 1) / 2]) {
+    for (; kk + 2 <= ke; kk += 2) {
+        const double2 p0 = sp[kk], p1 = sp[kk + 1];
+        fold_bin_add<R, SHARE_P, PZ>(p0, invP, cc, nphi_d, negn, ls, hb);
+        fold_bin_add<R, SHARE_P, PZ>(p1, invP, cc, nphi_d, negn, ls, hb);
+    }
+    if (kk < ke) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, ls, hb);
+}
+
+// Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
+template <int R, bool SHARE_P>
+__device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ sp, int kk, const int ke,
+                                                   const double (&invP)[R], const double (&cc)[R], const int n_phi,
+                                                   const uint32_t ls, const uint32_t (&hb)[(R + 1) / 2]) {
+    for (; kk < ke; ++kk) {
+        const double2 p = sp[kk];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
+            red_add_u32(((uint32_t)j << ls) + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
+        }
+    }
+}
+
+// S4, first half: close magnitude bin `seg_i` -- read and clear this thread's column of the phase histogram, add it to
+// the phase marginal, accumulate sum_j L(n_ij).  One phase bin j, all R trials.
+template <int R, bool DUMP>
+__device__ __forceinline__ void close_bin(const int j, const bool fold_overflow, const int n_phi, const uint32_t ls,
+                                          const uint32_t (&hb)[(R + 1) / 2], uint32_t (&mg)[(R + 1) / 2],
+                                          int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
+                                          const int lc, const int64_t s0, const bool (&valid)[R], const int seg_i) {
+    constexpr int RW = (R + 1) / 2;
+#pragma unroll
+    for (int w2 = 0; w2 < RW; ++w2) {
+        const uint32_t addr = hb[w2] + ((uint32_t)j << ls);
+        uint32_t w = lds_u32(addr);
+        sts_u32(addr, 0u);
+        if (fold_overflow) {  // j == 0: take over the counts of the overflow row n_phi
+            const uint32_t oaddr = hb[w2] + ((uint32_t)n_phi << ls);
+            w += lds_u32(oaddr);
+            sts_u32(oaddr, 0u);
+        }
+        mg[w2] += w;
+        const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
+        S2[2 * w2] += ltab_at(sL, prm.ltab, c0);
+        if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at(sL, prm.ltab, c1);
+        if (DUMP) {
+            if (valid[2 * w2])
+                prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
+            if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
+                prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * prm.n_m + seg_i] = c1;
+        }
+    }
+}
+
+// NPHI > 0: compile-time n_phi, 512 threads, phase marginal in registers.  NPHI == 0: any n_phi <= 64, threads per CTA
+// = 1 << prm.log2nt, marginal in shared memory.  R = trials per thread.  SHARE_P: the R trials of a thread share one
+// period (n_pdot % R == 0).  DUMP: test mode, trials come from a list and the count tables are written out.
+template <int NPHI, int R, bool SHARE_P, bool DUMP>
+__global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
     constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
+    constexpr bool REGM = NPHI > 0;
+    constexpr int NPHI_REG = REGM ? NPHI : 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int NT = blockDim.x, NW = NT >> 5;
     const int tid = threadIdx.x, lane = tid & 31;
-    const int n_phi = prm.n_phi, n_m = prm.n_m;
+    const int n_phi = REGM ? NPHI : prm.n_phi, n_m = prm.n_m;
+    const uint32_t ls = (uint32_t)(REGM ? kFastLog2NT : prm.log2nt) + 2u;  // log2(bytes between phase bins)
 
     // shared-memory carve-up
-    double2 *spts = reinterpret_cast<double2 *>(smem_raw);                                    // [kStages][kChunk]
-    int64_t *sL = reinterpret_cast<int64_t *>(spts + kStages * kChunk);                       // [kLtabSmem]
-    uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);                            // [kStages]
-    int *done = reinterpret_cast<int *>(full + kStages);                                      // [kStages]
-    int *sseg = done + kStages + 1;                                                           // [n_m + 1] (<= 65)
-    uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 2);                // [n_phi][RW][NT]
-    uint32_t *marg = hist + (size_t)n_phi * RW * NT;                                          // [n_phi][RW][NT]
+    double2 *spts = reinterpret_cast<double2 *>(smem_raw);                       // [cap_points]
+    int64_t *sL = reinterpret_cast<int64_t *>(spts + prm.cap_points);            // [kLtabSmem]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);               // [2]
+    int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
+    uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 2);   // [RW][n_phi + 1][NT]
+    const uint32_t plane = (uint32_t)(n_phi + 1) * (uint32_t)NT * 4u;            // bytes per counter-word plane
+    const uint32_t marg_off = (uint32_t)RW * plane;                              // NPHI == 0: marg follows hist
 
     const int lc = blockIdx.x / prm.jobs_per_lc;
     const int job = blockIdx.x % prm.jobs_per_lc;
@@ -277,24 +387,31 @@ __global__ void __launch_bounds__(1024, 1) k_search(const SearchParams prm) {
     const int N = prm.info[lc].n;
     const double dt_max = prm.info[lc].dt_max;
     const double2 *gpts = prm.pts + prm.lc_offsets[lc];
-    const int n_chunks = (N + kChunk - 1) / kChunk;
-    const int total_seq = n_tiles * n_chunks;
+    const bool single = N <= prm.cap_points;            // the whole light curve stays resident for every tile
+    const int CH = single ? N : prm.cap_points / 2;     // else: streamed through two half buffers, per tile
+    const int n_chunks = N > 0 ? (N + CH - 1) / CH : 0;
+    const int total_seq = single ? n_chunks : n_tiles * n_chunks;
     const int64_t TILE = (int64_t)NT * R;
 
-    // ---- prologue: zero histograms, stage table / segments, start the TMA ring
-    for (int i = tid; i < n_phi * RW * NT * 2; i += NT) hist[i] = 0u;  // hist and marg are contiguous
+    auto issue_chunk = [&](int g) {  // thread 0 only: TMA bulk copy of sequence element g into its buffer
+        const int c = g % n_chunks, buf = single ? 0 : (g & 1);
+        const int cnt = min(CH, N - c * CH);
+        mbar_expect_tx(&full[buf], (uint32_t)cnt * 16u);
+        for (int o = 0; o < cnt; o += 2048)
+            tma_load_bulk(spts + (size_t)buf * CH + o, gpts + (size_t)c * CH + o, (uint32_t)min(2048, cnt - o) * 16u, &full[buf]);
+    };
+
+    // ---- prologue: zero histograms, stage table / segments, start the point loads
+    for (int i = tid; i < (REGM ? RW : 2 * RW) * (n_phi + 1) * NT; i += NT) hist[i] = 0u;
     for (int i = tid; i < kLtabSmem; i += NT) sL[i] = i < prm.ltab_n ? prm.ltab[i] : 0;
     for (int i = tid; i <= n_m; i += NT) sseg[i] = prm.seg[(int64_t)lc * (n_m + 1) + i];
     if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); done[s] = 0; }
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        for (int g = 0; g < kStages && g < total_seq; ++g) {
-            const int c = g % n_chunks;
-            const int cnt = min(kChunk, N - c * kChunk);
-            mbar_expect_tx(&full[g], (uint32_t)cnt * 16u);
-            tma_load_bulk(spts + g * kChunk, gpts + (size_t)c * kChunk, (uint32_t)cnt * 16u, &full[g]);
-        }
+        if (n_tiles > 0)
+            for (int g = 0; g < 2 && g < total_seq; ++g) issue_chunk(g);
     }
     __syncthreads();
 
@@ -302,19 +419,25 @@ __global__ void __launch_bounds__(1024, 1) k_search(const SearchParams prm) {
     top.reset(prm.top_k > 0 ? prm.top_k : 1);
 
     const double nphi_d = (double)n_phi;
-    const double magic_b = kMagic + (double)prm.mod_bias;  // exact integer: floor(y) + bias in the low word
-    const uint32_t mod_mul = prm.mod_mul;
-    const uint32_t jstride = (uint32_t)(RW * NT) * 4u;     // bytes between consecutive phase bins
-    const uint32_t hbase = smem_u32(hist) + (uint32_t)tid * 4u;
+    const uint32_t negn = 0u - (uint32_t)n_phi;
+    uint32_t hb[RW];
+#pragma unroll
+    for (int w2 = 0; w2 < RW; ++w2) hb[w2] = smem_u32(hist) + (uint32_t)tid * 4u + (uint32_t)w2 * plane;
     const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)N : 0.0;
+    uint32_t mg[NPHI_REG][RW];  // phase marginal n_j of the R trials (NPHI > 0), packed like the histogram
+#pragma unroll
+    for (int j = 0; j < NPHI_REG; ++j)
+#pragma unroll
+        for (int w2 = 0; w2 < RW; ++w2) mg[j][w2] = 0u;
 
-    int g = 0;  // position in this CTA's chunk sequence
+    int g = 0;  // position in this CTA's chunk sequence (streamed mode)
     for (int tl = 0; tl < n_tiles; ++tl) {
         const int64_t s0 = (tile_lo + tl) * TILE + (int64_t)tid * R;  // first trial slot of this thread
         // ---- per-trial constants
         double invP[R], cc[R];  // SHARE_P: only invP[0] is used
         int64_t qv[R];
         bool valid[R];
+        bool fast = true, pz = true;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int64_t s = s0 + r;
@@ -323,159 +446,122 @@ __global__ void __launch_bounds__(1024, 1) k_search(const SearchParams prm) {
             if (valid[r]) q = DUMP ? prm.trial_q[s] : s;
             qv[r] = q;
             double ip = 0.0, c = 0.0;
-            if (valid[r]) trial_constants(prm.periods[q / prm.n_pdot], prm.pdots[q % prm.n_pdot], ip, c);
+            if (valid[r] && (!SHARE_P || r == 0)) ip = __ddiv_rn(1.0, prm.periods[q / prm.n_pdot]);
+            if (SHARE_P && r > 0) ip = invP[0];
+            if (valid[r]) c = __dmul_rn(__dmul_rn(__dmul_rn(-0.5, prm.pdots[q % prm.n_pdot]), ip), ip);
             invP[r] = ip;
             cc[r] = c;
-        }
-        // can this warp use the 32-bit floor/mod fast path for every point? (conservative bound on |y|)
-        bool fast = true;
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const double ip = invP[SHARE_P ? 0 : r];
-            const double yb = nphi_d * (dt_max * fabs(ip) + dt_max * dt_max * fabs(cc[r])) * 1.000001;
-            fast = fast && (yb < prm.y_safe);
+            // conservative bound on |y|: below 2^51 the magic-add floors are exact
+            fast = fast && (nphi_d * (dt_max * fabs(ip) + dt_max * dt_max * fabs(c)) * 1.000001 < kYSafe);
+            pz = pz && (c == 0.0);
         }
         fast = __all_sync(0xffffffffu, fast);
+        pz = __all_sync(0xffffffffu, pz);
 
         int64_t S2[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) S2[r] = 0;
 
         int seg_i = 0;  // current magnitude bin
-        for (int c = 0; c < n_chunks; ++c, ++g) {
-            const int slot = g % kStages;
-            mbar_wait(&full[slot], (uint32_t)((g / kStages) & 1));
-            const double2 *sp = spts + slot * kChunk;
-            const int k_base = c * kChunk;
-            const int k_end = min(N, k_base + kChunk);
+        for (int c = 0; c < n_chunks; ++c) {
+            const int buf = single ? 0 : (g & 1);
+            if (!single || tl == 0) mbar_wait(&full[buf], single ? 0u : (uint32_t)((g >> 1) & 1));
+            const double2 *sp = spts + (size_t)buf * CH;
+            const int k_base = c * CH;
+            const int k_end = min(N, k_base + CH);
             int k = k_base;
             while (k < k_end) {
                 const int e = min(k_end, sseg[seg_i + 1]);
                 // ---------------- hot loop: fold + bin the points [k, e) of magnitude bin seg_i
                 if (fast) {
-                    // points are loaded in groups of kUnroll before any histogram update of the group, so the
-                    // broadcast LDS.128 of a group overlap (the updates are "memory"-clobbering asm)
-                    auto fold_bin_add = [&](const double2 p) {
-                        double a;
-                        if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
-                            const double b = __dmul_rn(p.y, cc[r]);
-                            const double x = __dadd_rn(a, b);
-                            const double y = __dmul_rn(x, nphi_d);
-                            const double z = __dadd_rd(y, magic_b);
-                            const uint32_t Iu = (uint32_t)__double2loint(z);      // floor(y) + bias >= 0
-                            const uint32_t qd = __umulhi(Iu, mod_mul);             // Iu / n_phi
-                            const uint32_t j = Iu - qd * (uint32_t)n_phi;          // Iu mod n_phi
-                            const uint32_t addr = hbase + j * jstride + (uint32_t)(r >> 1) * (uint32_t)NT * 4u;
-                            const uint32_t inc = (r & 1) ? 0x10000u : 1u;
-#if GCE_HIST_ATOMIC
-                            asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(inc) : "memory");
-#else
-                            uint32_t w;
-                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(addr) : "memory");
-                            w += inc;
-                            asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(w) : "memory");
-#endif
-                        }
-                    };
-                    int kk = k - k_base;
-                    const int ke = e - k_base;
-                    for (; kk + kUnroll <= ke; kk += kUnroll) {
-                        double2 p[kUnroll];
-#pragma unroll
-                        for (int u = 0; u < kUnroll; ++u) p[u] = sp[kk + u];
-#pragma unroll
-                        for (int u = 0; u < kUnroll; ++u) fold_bin_add(p[u]);
-                    }
-                    for (; kk < ke; ++kk) fold_bin_add(sp[kk]);
+                    if (pz) fold_range<R, SHARE_P, true>(sp, k - k_base, e - k_base, invP, cc, nphi_d, negn, ls, hb);
+                    else fold_range<R, SHARE_P, false>(sp, k - k_base, e - k_base, invP, cc, nphi_d, negn, ls, hb);
                 } else {
-                    for (int kk = k - k_base; kk < e - k_base; ++kk) {
-                        const double2 p = sp[kk];
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
-                            hist[((size_t)j * RW + (r >> 1)) * NT + tid] += (r & 1) ? 0x10000u : 1u;
-                        }
-                    }
+                    fold_range_generic<R, SHARE_P>(sp, k - k_base, e - k_base, invP, cc, n_phi, ls, hb);
                 }
                 k = e;
                 // ---------------- S4: close every magnitude bin that ends here (possibly several empty ones)
                 while (seg_i < n_m && sseg[seg_i + 1] == k) {
-                    for (int j = 0; j < n_phi; ++j) {
+                    if (sseg[seg_i + 1] > sseg[seg_i]) {
+                        if (REGM) {
 #pragma unroll
-                        for (int w2 = 0; w2 < RW; ++w2) {
-                            const size_t idx = ((size_t)j * RW + w2) * NT + tid;
-                            const uint32_t w = hist[idx];
-                            if (w) {
-                                hist[idx] = 0u;
-                                marg[idx] += w;
-                            }
-                            const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-                            S2[2 * w2] += c0 < kLtabSmem ? sL[c0] : prm.ltab[c0];
-                            if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += c1 < kLtabSmem ? sL[c1] : prm.ltab[c1];
-                            if (DUMP) {
-                                if (valid[2 * w2])
-                                    prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * n_m + seg_i] = c0;
-                                if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
-                                    prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * n_m + seg_i] = c1;
+                            for (int j = 0; j < NPHI_REG; ++j)
+                                close_bin<R, DUMP>(j, j == 0, n_phi, ls, hb, mg[j], S2, sL, prm, lc, s0, valid, seg_i);
+                        } else {
+                            for (int j = 0; j < n_phi; ++j) {
+                                uint32_t m2[RW];
+#pragma unroll
+                                for (int w2 = 0; w2 < RW; ++w2) m2[w2] = lds_u32(hb[w2] + marg_off + ((uint32_t)j << ls));
+                                close_bin<R, DUMP>(j, j == 0, n_phi, ls, hb, m2, S2, sL, prm, lc, s0, valid, seg_i);
+#pragma unroll
+                                for (int w2 = 0; w2 < RW; ++w2) sts_u32(hb[w2] + marg_off + ((uint32_t)j << ls), m2[w2]);
                             }
                         }
                     }
                     ++seg_i;
                 }
             }
-            // ---------------- release the stage; the last warp to finish refills it (no dedicated producer)
-            __syncwarp();
-            if (lane == 0) {
-                __threadfence_block();
-                const int old = atomicAdd(&done[slot], 1);
-                if (old == NW - 1) {
-                    done[slot] = 0;
-                    const int gn = g + kStages;
-                    if (gn < total_seq) {
-                        const int cn = gn % n_chunks;
-                        const int cnt = min(kChunk, N - cn * kChunk);
-                        __threadfence_block();
-                        mbar_expect_tx(&full[slot], (uint32_t)cnt * 16u);
-                        tma_load_bulk(spts + slot * kChunk, gpts + (size_t)cn * kChunk, (uint32_t)cnt * 16u, &full[slot]);
-                    }
-                }
+            if (!single) {  // streamed mode: everyone is done with this half buffer -> refill it with element g + 2
+                __syncthreads();
+                if (tid == 0 && g + 2 < total_seq) issue_chunk(g + 2);
+                ++g;
             }
         }
-        // trailing empty magnitude bins when N == 0 never occur (n_chunks == 0); DUMP tables stay zeroed by caller
 
         // ---------------- finish the trials: S1 = sum_j L(n_j), CE, outputs
         int64_t S1[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) S1[r] = 0;
         if (N > 0) {
-            for (int j = 0; j < n_phi; ++j) {
+            auto add_marg = [&](const uint32_t w, const int w2) {
+                const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
+                S1[2 * w2] += ltab_at(sL, prm.ltab, c0);
+                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at(sL, prm.ltab, c1);
+            };
+            if (REGM) {
 #pragma unroll
-                for (int w2 = 0; w2 < RW; ++w2) {
-                    const size_t idx = ((size_t)j * RW + w2) * NT + tid;
-                    const uint32_t w = marg[idx];
-                    marg[idx] = 0u;
-                    const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-                    S1[2 * w2] += c0 < kLtabSmem ? sL[c0] : prm.ltab[c0];
-                    if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += c1 < kLtabSmem ? sL[c1] : prm.ltab[c1];
-                }
+                for (int j = 0; j < NPHI_REG; ++j)
+#pragma unroll
+                    for (int w2 = 0; w2 < RW; ++w2) { add_marg(mg[j][w2], w2); mg[j][w2] = 0u; }
+            } else {
+                for (int j = 0; j < n_phi; ++j)
+#pragma unroll
+                    for (int w2 = 0; w2 < RW; ++w2) {
+                        const uint32_t addr = hb[w2] + marg_off + ((uint32_t)j << ls);
+                        add_marg(lds_u32(addr), w2);
+                        sts_u32(addr, 0u);
+                    }
             }
         }
+        double ce[R];
+        int64_t S[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t S = S1[r] - S2[r];  // = N * CE * 2^42, exact
-            const double ce = N > 0 ? (double)S * ce_scale : CUDART_NAN;
-            if (DUMP) {
-                if (valid[r] && prm.out_ce_at) prm.out_ce_at[(int64_t)lc * prm.n_trials + s0 + r] = ce;
-            } else {
-                if (valid[r] && prm.out_ce) {
-                    const int64_t o = (int64_t)lc * prm.n_trials + qv[r];
-                    if (prm.ce_fp64) reinterpret_cast<double *>(prm.out_ce)[o] = ce;
-                    else reinterpret_cast<float *>(prm.out_ce)[o] = (float)ce;
+            S[r] = S1[r] - S2[r];  // = N * CE * 2^42, exact
+            ce[r] = N > 0 ? (double)S[r] * ce_scale : CUDART_NAN;
+        }
+        if (DUMP) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (valid[r] && prm.out_ce_at) prm.out_ce_at[(int64_t)lc * prm.n_trials + s0 + r] = ce[r];
+        } else {
+            if (prm.out_ce) {
+                const int64_t o = (int64_t)lc * prm.n_trials + s0;  // q == slot outside DUMP
+                float *o32 = reinterpret_cast<float *>(prm.out_ce) + o;
+                if (R == 4 && !prm.ce_fp64 && valid[R - 1] && (reinterpret_cast<uintptr_t>(o32) & 15u) == 0) {
+                    *reinterpret_cast<float4 *>(o32) = make_float4((float)ce[0], (float)ce[1 % R], (float)ce[2 % R], (float)ce[3 % R]);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        if (!valid[r]) continue;
+                        if (prm.ce_fp64) reinterpret_cast<double *>(prm.out_ce)[o + r] = ce[r];
+                        else o32[r] = (float)ce[r];
+                    }
                 }
-                if (prm.top_k > 0) top.offer((valid[r] && N > 0) ? S : kInfS, (valid[r] && N > 0) ? qv[r] : kInfS);
+            }
+            if (prm.top_k > 0) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) top.offer((valid[r] && N > 0) ? S[r] : kInfS, (valid[r] && N > 0) ? qv[r] : kInfS);
             }
         }
     }
@@ -483,9 +569,8 @@ __global__ void __launch_bounds__(1024, 1) k_search(const SearchParams prm) {
     // ---------------- per-CTA merge of the warps' top-k lists -> partial[lc][job][k]
     if (!DUMP && prm.top_k > 0) {
         const int K = prm.top_k;
-        __syncthreads();  // every issued TMA load has been consumed: the point ring is idle, reuse it as scratch
-        static_assert(sizeof(double2) * kStages * kChunk >= 16 * 32 * GCE_CE_MAX_TOPK, "scratch too small");
-        int64_t *scr = reinterpret_cast<int64_t *>(spts);
+        __syncthreads();  // every issued TMA load has been consumed: the point buffer is idle, reuse it as scratch
+        int64_t *scr = reinterpret_cast<int64_t *>(spts);  // 16 * NW * K <= 8 KB <= cap_points * 16 (cap >= 512)
         if (lane < K) {
             scr[2 * ((tid >> 5) * K + lane)] = top.S;
             scr[2 * ((tid >> 5) * K + lane) + 1] = top.q;
@@ -575,28 +660,52 @@ thread_local int g_last_cuda_error = 0;
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-struct Layout {
-    size_t pts, seg, info, ltab, part_S, part_q, total;
-    int ltab_n;
-};
-
+// Which kernel variant runs, with how many threads, over how many CTAs: decided from sizes only (deterministic, no
+// device query), so gce_ce_workspace_bytes and gce_ce_search agree.
 struct Plan {
-    int R;
-    bool share_p;
+    int R;             // trials per thread
+    bool share_p;      // the R trials of a thread share one period
+    int nphi_t;        // compile-time n_phi of the kernel (15, 20, 30) or 0 = generic
+    int log2nt;        // threads per CTA = 1 << log2nt
+    int cap_points;    // shared-memory point buffer capacity
+    size_t smem;       // dynamic shared memory per CTA
     int64_t tiles_per_lc;
     int jobs_per_lc;
 };
 
-// Trials per thread and Pdot sharing: decided from sizes only (deterministic, no device query).
-Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int nt) {
+size_t search_smem_fixed() {
+    return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 2);
+}
+size_t search_smem_planes(int n_phi, int R, bool regm, int nt) {
+    const int RW = (R + 1) / 2;
+    return (size_t)(regm ? RW : 2 * RW) * (size_t)(n_phi + 1) * (size_t)nt * sizeof(uint32_t);
+}
+
+Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int n_phi, bool dump) {
     Plan p;
-    p.R = 2;
-    p.share_p = (n_pdot % p.R) == 0;
-    const int64_t tile = (int64_t)nt * p.R;
+    if (dump) { p.R = 2; p.share_p = false; }
+    else if (n_pdot % 4 == 0) { p.R = 4; p.share_p = true; }
+    else if (n_pdot % 2 == 0) { p.R = 2; p.share_p = true; }
+    else { p.R = 4; p.share_p = false; }
+    const size_t fixed = search_smem_fixed();
+    const size_t min_pts = 512 * sizeof(double2);  // also the top-k merge scratch
+    p.nphi_t = 0;
+    if (!dump && (n_phi == 15 || n_phi == 20 || n_phi == 30) &&
+        fixed + search_smem_planes(n_phi, p.R, true, 1 << kFastLog2NT) + min_pts <= (size_t)kSmemLimit)
+        p.nphi_t = n_phi;
+    p.log2nt = kFastLog2NT;
+    if (p.nphi_t == 0)
+        while (p.log2nt > 5 && fixed + search_smem_planes(n_phi, p.R, false, 1 << p.log2nt) + min_pts > (size_t)kSmemLimit) --p.log2nt;
+    const size_t planes = search_smem_planes(n_phi, p.R, p.nphi_t != 0, 1 << p.log2nt);
+    int64_t cap = ((int64_t)kSmemLimit - (int64_t)fixed - (int64_t)planes) / (int64_t)sizeof(double2);
+    cap = cap / 8 * 8;
+    if (cap > 8192) cap = 8192;  // 128 KB of points; longer light curves are streamed
+    p.cap_points = (int)cap;
+    p.smem = (size_t)cap * sizeof(double2) + fixed + planes;
+    const int64_t tile = (int64_t)(1 << p.log2nt) * p.R;
     p.tiles_per_lc = n_trials > 0 ? (n_trials + tile - 1) / tile : 0;
-    // ~16 CTAs per SM-slot overall for dynamic balance, at least one tile per job
+    // ~16 CTAs per SM overall for dynamic balance, at least one tile per job
     int64_t want = (148LL * 16 + (n_lc > 0 ? n_lc : 1) - 1) / (n_lc > 0 ? n_lc : 1);
-    if (want < 1) want = 1;
     if (want > p.tiles_per_lc) want = p.tiles_per_lc;
     if (want < 1) want = 1;
     if (want > 4096) want = 4096;
@@ -604,9 +713,12 @@ Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int nt) {
     return p;
 }
 
-constexpr int kPlanThreads = 512;  // threads per CTA assumed by the workspace plan (kernel may run fewer CTAs/SM)
+struct Layout {
+    size_t pts, seg, info, ltab, part_S, part_q, total;
+    int ltab_n;
+};
 
-Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t n_pdot, const gce_ce_params *prm) {
+Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t n_pdot, const gce_ce_params *prm, bool dump) {
     Layout L;
     size_t o = 0;
     L.pts = o; o = align_up(o + sizeof(double2) * (size_t)(total_points > 0 ? total_points : 1), 256);
@@ -615,7 +727,7 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     int64_t tn = total_points < GCE_CE_MAX_POINTS ? total_points : GCE_CE_MAX_POINTS;
     L.ltab_n = (int)tn + 1;
     L.ltab = o; o = align_up(o + sizeof(int64_t) * (size_t)L.ltab_n, 256);
-    const Plan p = make_plan(n_lc, n_trials, n_pdot, kPlanThreads);
+    const Plan p = make_plan(n_lc, n_trials, n_pdot, prm->n_phase_bins, dump);
     const size_t parts = (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc * (size_t)(prm->top_k > 0 ? prm->top_k : 1);
     L.part_S = o; o = align_up(o + sizeof(int64_t) * parts, 256);
     L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
@@ -659,50 +771,33 @@ int cuda_fail(cudaError_t e) {
     return GCE_CE_ERR_CUDA;
 }
 
-size_t search_smem_bytes(int nt, int n_phi, int R) {
-    const int RW = (R + 1) / 2;
-    size_t fixed = sizeof(double2) * kStages * kChunk + sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * kStages +
-                   sizeof(int) * (kStages + 1) + sizeof(int) * (GCE_CE_MAX_BINS + 2);
-    return fixed + (size_t)2 * n_phi * RW * nt * sizeof(uint32_t);
-}
-
-template <int R, bool SHARE_P, bool DUMP>
-int launch_search(const SearchParams &sp, int32_t n_lc, cudaStream_t st) {
-    auto kern = k_search<R, SHARE_P, DUMP>;
-    // choose threads per CTA: the most resident threads per SM that registers and shared memory allow
-    int best_nt = 0, best_threads = 0;
-    const int cands[] = {1024, 768, 512, 384, 256, 128, 64, 32};
-    for (int nt : cands) {
-        const size_t smem = search_smem_bytes(nt, sp.n_phi, R);
-        if (smem > 227 * 1024) continue;
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
-            cudaGetLastError();
-            continue;
-        }
-        int blocks = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks, kern, nt, smem) != cudaSuccess) {
-            cudaGetLastError();
-            continue;
-        }
-        if (blocks * nt > best_threads) { best_threads = blocks * nt; best_nt = nt; }
-    }
-    if (best_nt == 0) return GCE_CE_ERR_RANGE;
-    // the workspace plan (partials) was sized for kPlanThreads; a smaller CTA would need more tiles per job, which
-    // is fine (jobs_per_lc is fixed by the plan), a larger one fewer.
-    SearchParams p = sp;
-    const int64_t tile = (int64_t)best_nt * R;
-    p.tiles_per_lc = p.n_trials > 0 ? (p.n_trials + tile - 1) / tile : 0;
-    if (p.jobs_per_lc > p.tiles_per_lc) {
-        // fewer tiles than planned jobs: surplus jobs get empty tile ranges (they still write +inf partials)
-    }
-    const size_t smem = search_smem_bytes(best_nt, p.n_phi, R);
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+template <int NPHI, int R, bool SHARE_P, bool DUMP>
+int launch_search(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
+    auto kern = k_search<NPHI, R, SHARE_P, DUMP>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem);
     if (e != cudaSuccess) return cuda_fail(e);
-    const unsigned grid = (unsigned)((int64_t)n_lc * p.jobs_per_lc);
-    kern<<<grid, best_nt, smem, st>>>(p);
+    const unsigned grid = (unsigned)((int64_t)n_lc * plan.jobs_per_lc);
+    kern<<<grid, 1 << plan.log2nt, plan.smem, st>>>(sp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return GCE_CE_OK;
+}
+
+template <int NPHI>
+int launch_search_variant(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
+    if (plan.share_p && plan.R == 4) return launch_search<NPHI, 4, true, false>(sp, plan, n_lc, st);
+    if (plan.share_p && plan.R == 2) return launch_search<NPHI, 2, true, false>(sp, plan, n_lc, st);
+    return launch_search<NPHI, 4, false, false>(sp, plan, n_lc, st);
+}
+
+int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t n_lc, cudaStream_t st) {
+    if (dump) return launch_search<0, 2, false, true>(sp, plan, n_lc, st);
+    switch (plan.nphi_t) {
+        case 15: return launch_search_variant<15>(sp, plan, n_lc, st);
+        case 20: return launch_search_variant<20>(sp, plan, n_lc, st);
+        case 30: return launch_search_variant<30>(sp, plan, n_lc, st);
+        default: return launch_search_variant<0>(sp, plan, n_lc, st);
+    }
 }
 
 }  // namespace
@@ -737,7 +832,7 @@ int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int6
     if (rc) return rc;
     rc = check_sizes(n_lc, total_points, n_p, n_pdot);
     if (rc) return rc;
-    *bytes = make_layout(total_points, n_lc, n_p * n_pdot, n_pdot, prm).total;
+    *bytes = make_layout(total_points, n_lc, n_p * n_pdot, n_pdot, prm, false).total;
     return GCE_CE_OK;
 }
 
@@ -765,7 +860,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     const int64_t n_trials = dump ? n_dump : n_p * n_pdot;
     gce_ce_params lay_prm = *prm;
     if (dump) lay_prm.top_k = 0;
-    const Layout L = make_layout(total_points, n_lc, n_trials, dump ? 1 : n_pdot, &lay_prm);
+    const Layout L = make_layout(total_points, n_lc, n_trials, dump ? 1 : n_pdot, &lay_prm, dump);
     if (workspace_bytes < L.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return GCE_CE_ERR_WORKSPACE;
     if (n_lc == 0) return GCE_CE_OK;
 
@@ -783,15 +878,17 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
 
-    const Plan plan = make_plan(n_lc, n_trials, dump ? 1 : n_pdot, kPlanThreads);
+    const Plan plan = make_plan(n_lc, n_trials, dump ? 1 : n_pdot, prm->n_phase_bins, dump);
     SearchParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.pts = pts; sp.seg = seg; sp.info = info; sp.lc_offsets = lc_offsets; sp.ltab = ltab;
     sp.periods = periods; sp.pdots = pdots; sp.trial_q = trial_q;
     sp.n_p = n_p; sp.n_pdot = n_pdot; sp.n_trials = n_trials;
     sp.jobs_per_lc = plan.jobs_per_lc;
+    sp.tiles_per_lc = plan.tiles_per_lc;
+    sp.log2nt = plan.log2nt;
+    sp.cap_points = plan.cap_points;
     sp.n_phi = prm->n_phase_bins; sp.n_m = prm->n_mag_bins;
-    mod_constants(prm->n_phase_bins, &sp.mod_mul, &sp.mod_bias, &sp.y_safe);
     sp.ltab_n = L.ltab_n;
     sp.top_k = dump ? 0 : prm->top_k;
     sp.ce_fp64 = prm->ce_fp64;
@@ -805,9 +902,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
         if (e != cudaSuccess) return cuda_fail(e);
     }
     if (n_trials > 0) {
-        if (dump) rc = launch_search<2, false, true>(sp, n_lc, st);
-        else if (plan.share_p) rc = launch_search<2, true, false>(sp, n_lc, st);
-        else rc = launch_search<2, false, false>(sp, n_lc, st);
+        rc = dispatch_search(sp, plan, dump, n_lc, st);
         if (rc) return rc;
     }
     if (prm->ev_search_end) {
