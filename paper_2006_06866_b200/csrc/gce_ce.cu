@@ -45,6 +45,9 @@ constexpr int64_t kInfS = INT64_MAX;
 constexpr int kSmemLimit = 227 * 1024;
 constexpr int kFastLog2NT = 9;    // the compile-time-n_phi kernels run 512 threads per CTA
 
+struct FalseT { static constexpr bool value = false; };
+struct TrueT { static constexpr bool value = true; };
+
 struct LcInfo {
     int32_t n;
     int32_t pad;
@@ -266,8 +269,19 @@ __device__ __forceinline__ void red_add_u32(uint32_t addr, uint32_t inc) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(inc) : "memory");
 }
 
-// L(k) = k ln k in 2^-42 fixed point: first kLtabSmem entries from shared memory, the (rare) rest from global.
+// read-and-clear of one counter word in one LSU instruction (ATOMS.EXCH)
+__device__ __forceinline__ uint32_t exch0_u32(uint32_t addr) {
+    uint32_t w;
+    asm volatile("atom.shared.exch.b32 %0, [%1], %2;" : "=r"(w) : "r"(addr), "r"(0u) : "memory");
+    return w;
+}
+
+// L(k) = k ln k in 2^-42 fixed point.  BIG = false: the caller guarantees c < kLtabSmem (a bound on the number of
+// points that can be in the cell), one LDS.64.  BIG = true: first kLtabSmem entries from shared memory, the rest
+// from global.
+template <bool BIG>
 __device__ __forceinline__ int64_t ltab_at(const int64_t *__restrict__ sL, const int64_t *__restrict__ gL, uint32_t c) {
+    if (!BIG) return sL[c];
     int64_t v = sL[c & (kLtabSmem - 1)];
     if (c >= (uint32_t)kLtabSmem) v = gL[c];
     return v;
@@ -327,7 +341,7 @@ __device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ s
 
 // S4, first half: close magnitude bin `seg_i` -- read and clear this thread's column of the phase histogram, add it to
 // the phase marginal, accumulate sum_j L(n_ij).  One phase bin j, all R trials.
-template <int R, bool DUMP>
+template <int R, bool DUMP, bool BIG>
 __device__ __forceinline__ void close_bin(const int j, const bool fold_overflow, const int n_phi, const uint32_t ls,
                                           const uint32_t (&hb)[(R + 1) / 2], uint32_t (&mg)[(R + 1) / 2],
                                           int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
@@ -335,23 +349,41 @@ __device__ __forceinline__ void close_bin(const int j, const bool fold_overflow,
     constexpr int RW = (R + 1) / 2;
 #pragma unroll
     for (int w2 = 0; w2 < RW; ++w2) {
-        const uint32_t addr = hb[w2] + ((uint32_t)j << ls);
-        uint32_t w = lds_u32(addr);
-        sts_u32(addr, 0u);
-        if (fold_overflow) {  // j == 0: take over the counts of the overflow row n_phi
-            const uint32_t oaddr = hb[w2] + ((uint32_t)n_phi << ls);
-            w += lds_u32(oaddr);
-            sts_u32(oaddr, 0u);
-        }
+        uint32_t w = exch0_u32(hb[w2] + ((uint32_t)j << ls));
+        if (fold_overflow) w += exch0_u32(hb[w2] + ((uint32_t)n_phi << ls));  // j == 0 takes over the overflow row
         mg[w2] += w;
         const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-        S2[2 * w2] += ltab_at(sL, prm.ltab, c0);
-        if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at(sL, prm.ltab, c1);
+        S2[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
+        if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
         if (DUMP) {
             if (valid[2 * w2])
                 prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
             if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
                 prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * prm.n_m + seg_i] = c1;
+        }
+    }
+}
+
+// All phase bins of magnitude bin seg_i.  MG: phase marginal, registers (NPHI > 0) or shared memory (NPHI == 0).
+template <int NPHI, int R, bool DUMP, bool BIG>
+__device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t ls, const uint32_t marg_off,
+                                              const uint32_t (&hb)[(R + 1) / 2],
+                                              uint32_t (&mg)[NPHI > 0 ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
+                                              const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
+                                              const int64_t s0, const bool (&valid)[R], const int seg_i) {
+    constexpr int RW = (R + 1) / 2;
+    if (NPHI > 0) {
+#pragma unroll
+        for (int j = 0; j < (NPHI > 0 ? NPHI : 1); ++j)
+            close_bin<R, DUMP, BIG>(j, j == 0, n_phi, ls, hb, mg[j], S2, sL, prm, lc, s0, valid, seg_i);
+    } else {
+        for (int j = 0; j < n_phi; ++j) {
+            uint32_t m2[RW];
+#pragma unroll
+            for (int w2 = 0; w2 < RW; ++w2) m2[w2] = lds_u32(hb[w2] + marg_off + ((uint32_t)j << ls));
+            close_bin<R, DUMP, BIG>(j, j == 0, n_phi, ls, hb, m2, S2, sL, prm, lc, s0, valid, seg_i);
+#pragma unroll
+            for (int w2 = 0; w2 < RW; ++w2) sts_u32(hb[w2] + marg_off + ((uint32_t)j << ls), m2[w2]);
         }
     }
 }
@@ -370,14 +402,15 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
     const int n_phi = REGM ? NPHI : prm.n_phi, n_m = prm.n_m;
     const uint32_t ls = (uint32_t)(REGM ? kFastLog2NT : prm.log2nt) + 2u;  // log2(bytes between phase bins)
 
-    // shared-memory carve-up
-    double2 *spts = reinterpret_cast<double2 *>(smem_raw);                       // [cap_points]
-    int64_t *sL = reinterpret_cast<int64_t *>(spts + prm.cap_points);            // [kLtabSmem]
+    // shared-memory carve-up: the L table first (compile-time offset, so lookups are LDS.64 [c*8 + imm]), points last
+    int64_t *sL = reinterpret_cast<int64_t *>(smem_raw);                         // [kLtabSmem]
     uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);               // [2]
     int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
-    uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 2);   // [RW][n_phi + 1][NT]
+    uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 4);   // [RW][n_phi + 1][NT], 16-byte aligned
     const uint32_t plane = (uint32_t)(n_phi + 1) * (uint32_t)NT * 4u;            // bytes per counter-word plane
     const uint32_t marg_off = (uint32_t)RW * plane;                              // NPHI == 0: marg follows hist
+    double2 *spts = reinterpret_cast<double2 *>(reinterpret_cast<unsigned char *>(hist) +
+                                                (size_t)(REGM ? RW : 2 * RW) * plane);  // [cap_points]
 
     const int lc = blockIdx.x / prm.jobs_per_lc;
     const int job = blockIdx.x % prm.jobs_per_lc;
@@ -430,6 +463,14 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
 #pragma unroll
         for (int w2 = 0; w2 < RW; ++w2) mg[j][w2] = 0u;
 
+    // Warps that share an SM sub-partition (warp id mod 4) start at different magnitude bins, a quarter of the points
+    // apart, so that one warp's S4 (no FP64) overlaps the others' folds (FP64-bound).  Counts and the integer entropy
+    // sums do not depend on the order of the bins.  Streamed light curves are processed in storage order.
+    int rot = 0;
+    if (single && n_m > 1) {
+        const int target = (int)(((int64_t)N * ((tid >> 7) & 3)) >> 2);
+        while (rot + 1 < n_m && sseg[rot + 1] <= target) ++rot;
+    }
     int g = 0;  // position in this CTA's chunk sequence (streamed mode)
     for (int tl = 0; tl < n_tiles; ++tl) {
         const int64_t s0 = (tile_lo + tl) * TILE + (int64_t)tid * R;  // first trial slot of this thread
@@ -462,44 +503,36 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
 #pragma unroll
         for (int r = 0; r < R; ++r) S2[r] = 0;
 
-        int seg_i = 0;  // current magnitude bin
+        int seg_s = 0;  // magnitude bins finished so far, counted in this warp's (rotated) order
         for (int c = 0; c < n_chunks; ++c) {
             const int buf = single ? 0 : (g & 1);
             if (!single || tl == 0) mbar_wait(&full[buf], single ? 0u : (uint32_t)((g >> 1) & 1));
             const double2 *sp = spts + (size_t)buf * CH;
             const int k_base = c * CH;
             const int k_end = min(N, k_base + CH);
-            int k = k_base;
-            while (k < k_end) {
-                const int e = min(k_end, sseg[seg_i + 1]);
-                // ---------------- hot loop: fold + bin the points [k, e) of magnitude bin seg_i
-                if (fast) {
-                    if (pz) fold_range<R, SHARE_P, true>(sp, k - k_base, e - k_base, invP, cc, nphi_d, negn, ls, hb);
-                    else fold_range<R, SHARE_P, false>(sp, k - k_base, e - k_base, invP, cc, nphi_d, negn, ls, hb);
-                } else {
-                    fold_range_generic<R, SHARE_P>(sp, k - k_base, e - k_base, invP, cc, n_phi, ls, hb);
-                }
-                k = e;
-                // ---------------- S4: close every magnitude bin that ends here (possibly several empty ones)
-                while (seg_i < n_m && sseg[seg_i + 1] == k) {
-                    if (sseg[seg_i + 1] > sseg[seg_i]) {
-                        if (REGM) {
-#pragma unroll
-                            for (int j = 0; j < NPHI_REG; ++j)
-                                close_bin<R, DUMP>(j, j == 0, n_phi, ls, hb, mg[j], S2, sL, prm, lc, s0, valid, seg_i);
-                        } else {
-                            for (int j = 0; j < n_phi; ++j) {
-                                uint32_t m2[RW];
-#pragma unroll
-                                for (int w2 = 0; w2 < RW; ++w2) m2[w2] = lds_u32(hb[w2] + marg_off + ((uint32_t)j << ls));
-                                close_bin<R, DUMP>(j, j == 0, n_phi, ls, hb, m2, S2, sL, prm, lc, s0, valid, seg_i);
-#pragma unroll
-                                for (int w2 = 0; w2 < RW; ++w2) sts_u32(hb[w2] + marg_off + ((uint32_t)j << ls), m2[w2]);
-                            }
-                        }
+            while (seg_s < n_m) {
+                int seg_i = seg_s + rot;
+                if (seg_i >= n_m) seg_i -= n_m;
+                const int b0 = sseg[seg_i], b1 = sseg[seg_i + 1];
+                const int lo = max(b0, k_base) - k_base, hi = min(b1, k_end) - k_base;
+                // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
+                if (lo < hi) {
+                    if (fast) {
+                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, ls, hb);
+                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, ls, hb);
+                    } else {
+                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, ls, hb);
                     }
-                    ++seg_i;
                 }
+                if (b1 > k_end) break;  // the bin continues in the next buffer
+                // ---------------- S4: the bin is complete; a cell holds at most b1 - b0 points
+                if (b1 > b0) {
+                    if (b1 - b0 < kLtabSmem)
+                        close_mag_bin<NPHI, R, DUMP, false>(n_phi, ls, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                    else
+                        close_mag_bin<NPHI, R, DUMP, true>(n_phi, ls, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                }
+                ++seg_s;
             }
             if (!single) {  // streamed mode: everyone is done with this half buffer -> refill it with element g + 2
                 __syncthreads();
@@ -513,25 +546,25 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
 #pragma unroll
         for (int r = 0; r < R; ++r) S1[r] = 0;
         if (N > 0) {
-            auto add_marg = [&](const uint32_t w, const int w2) {
+            auto add_marg = [&](const uint32_t w, const int w2, auto big) {
+                constexpr bool BIG = decltype(big)::value;
                 const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-                S1[2 * w2] += ltab_at(sL, prm.ltab, c0);
-                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at(sL, prm.ltab, c1);
+                S1[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
+                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
             };
-            if (REGM) {
+            auto marg_pass = [&](auto big) {
+                if (REGM) {
 #pragma unroll
-                for (int j = 0; j < NPHI_REG; ++j)
+                    for (int j = 0; j < NPHI_REG; ++j)
 #pragma unroll
-                    for (int w2 = 0; w2 < RW; ++w2) { add_marg(mg[j][w2], w2); mg[j][w2] = 0u; }
-            } else {
-                for (int j = 0; j < n_phi; ++j)
+                        for (int w2 = 0; w2 < RW; ++w2) { add_marg(mg[j][w2], w2, big); mg[j][w2] = 0u; }
+                } else {
+                    for (int j = 0; j < n_phi; ++j)
 #pragma unroll
-                    for (int w2 = 0; w2 < RW; ++w2) {
-                        const uint32_t addr = hb[w2] + marg_off + ((uint32_t)j << ls);
-                        add_marg(lds_u32(addr), w2);
-                        sts_u32(addr, 0u);
-                    }
-            }
+                        for (int w2 = 0; w2 < RW; ++w2) add_marg(exch0_u32(hb[w2] + marg_off + ((uint32_t)j << ls)), w2, big);
+                }
+            };
+            if (N < kLtabSmem) marg_pass(FalseT{}); else marg_pass(TrueT{});
         }
         double ce[R];
         int64_t S[R];
@@ -674,7 +707,7 @@ struct Plan {
 };
 
 size_t search_smem_fixed() {
-    return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 2);
+    return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4);
 }
 size_t search_smem_planes(int n_phi, int R, bool regm, int nt) {
     const int RW = (R + 1) / 2;
