@@ -311,17 +311,28 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
     }
 }
 
-// Hot loop over the points [kk, ke) of one shared-memory buffer (all of one magnitude bin).
+// Hot loop over the points [kk, ke) of one shared-memory buffer (all of one magnitude bin).  The next two points are
+// loaded before the current two are folded (the RED asm statements are compiler barriers, so the loads would otherwise
+// sit behind the previous iteration's atomics and the first DMUL would wait for them); the last trip reads up to two
+// entries past ke, which are inside the buffer's slack and never used.
 template <int R, bool SHARE_P, bool PZ>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
                                            const uint32_t ls, const uint32_t (&hb)[(R + 1) / 2]) {
-    for (; kk + 2 <= ke; kk += 2) {
-        const double2 p0 = sp[kk], p1 = sp[kk + 1];
-        fold_bin_add<R, SHARE_P, PZ>(p0, invP, cc, nphi_d, negn, ls, hb);
-        fold_bin_add<R, SHARE_P, PZ>(p1, invP, cc, nphi_d, negn, ls, hb);
+    if (ke - kk >= 4) {
+        double2 a0 = sp[kk], a1 = sp[kk + 1];
+        do {
+            const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
+            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, ls, hb);
+            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, ls, hb);
+            a0 = sp[kk + 4];
+            a1 = sp[kk + 5];
+            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, ls, hb);
+            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, ls, hb);
+            kk += 4;
+        } while (ke - kk >= 4);
     }
-    if (kk < ke) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, ls, hb);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, ls, hb);
 }
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
@@ -721,7 +732,7 @@ Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int n_phi, bool d
     else if (n_pdot % 2 == 0) { p.R = 2; p.share_p = true; }
     else { p.R = 4; p.share_p = false; }
     const size_t fixed = search_smem_fixed();
-    const size_t min_pts = 512 * sizeof(double2);  // also the top-k merge scratch
+    const size_t min_pts = (512 + 2) * sizeof(double2);  // also the top-k merge scratch
     p.nphi_t = 0;
     if (!dump && (n_phi == 15 || n_phi == 20 || n_phi == 30) &&
         fixed + search_smem_planes(n_phi, p.R, true, 1 << kFastLog2NT) + min_pts <= (size_t)kSmemLimit)
@@ -730,11 +741,11 @@ Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int n_phi, bool d
     if (p.nphi_t == 0)
         while (p.log2nt > 5 && fixed + search_smem_planes(n_phi, p.R, false, 1 << p.log2nt) + min_pts > (size_t)kSmemLimit) --p.log2nt;
     const size_t planes = search_smem_planes(n_phi, p.R, p.nphi_t != 0, 1 << p.log2nt);
-    int64_t cap = ((int64_t)kSmemLimit - (int64_t)fixed - (int64_t)planes) / (int64_t)sizeof(double2);
+    int64_t cap = ((int64_t)kSmemLimit - (int64_t)fixed - (int64_t)planes) / (int64_t)sizeof(double2) - 2;
     cap = cap / 8 * 8;
     if (cap > 8192) cap = 8192;  // 128 KB of points; longer light curves are streamed
     p.cap_points = (int)cap;
-    p.smem = (size_t)cap * sizeof(double2) + fixed + planes;
+    p.smem = (size_t)(cap + 2) * sizeof(double2) + fixed + planes;  // + 2: read-ahead slack of the hot loop
     const int64_t tile = (int64_t)(1 << p.log2nt) * p.R;
     p.tiles_per_lc = n_trials > 0 ? (n_trials + tile - 1) / tile : 0;
     // ~16 CTAs per SM overall for dynamic balance, at least one tile per job
