@@ -43,7 +43,7 @@ constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(
 constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
 constexpr int64_t kInfS = INT64_MAX;
 constexpr int kSmemLimit = 227 * 1024;
-constexpr int kFastLog2NT = 9;    // the compile-time-n_phi kernels run 512 threads per CTA
+constexpr int kCloseGroup = 5;    // phase bins whose read-and-clear atomics are in flight together in S4
 
 struct FalseT { static constexpr bool value = false; };
 struct TrueT { static constexpr bool value = true; };
@@ -67,7 +67,6 @@ struct SearchParams {
     int64_t tiles_per_lc;
     int32_t jobs_per_lc;
     int32_t n_phi, n_m;
-    int32_t log2nt;            // threads per CTA = 1 << log2nt
     int32_t cap_points;        // capacity of the shared-memory point buffer (multiple of 8)
     int32_t ltab_n;
     int32_t top_k;
@@ -257,14 +256,6 @@ __global__ void k_ltab(int64_t *__restrict__ ltab, int n) {
 }
 
 // ------------------------------------------------------------------------------------------------ S2..S5
-__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
-    uint32_t w;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(addr) : "memory");
-    return w;
-}
-__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t w) {
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(w) : "memory");
-}
 __device__ __forceinline__ void red_add_u32(uint32_t addr, uint32_t inc) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(inc) : "memory");
 }
@@ -295,7 +286,7 @@ __device__ __forceinline__ int64_t ltab_at(const int64_t *__restrict__ sL, const
 // PZ: every trial of the thread has c = +-0, so x = a bit for bit (a >= +0) and two operations are skipped.
 template <int R, bool SHARE_P, bool PZ>
 __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
-                                             const double nphi_d, const uint32_t negn, const uint32_t ls,
+                                             const double nphi_d, const uint32_t negn, const uint32_t rs,
                                              const uint32_t (&hb)[(R + 1) / 2]) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
@@ -307,7 +298,7 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
         const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
         const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
         const uint32_t j = Iy + Ix * negn;
-        red_add_u32((j << ls) + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
+        red_add_u32(j * rs + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
     }
 }
 
@@ -318,110 +309,130 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
 template <int R, bool SHARE_P, bool PZ>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
-                                           const uint32_t ls, const uint32_t (&hb)[(R + 1) / 2]) {
+                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2]) {
     if (ke - kk >= 4) {
         double2 a0 = sp[kk], a1 = sp[kk + 1];
         do {
             const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, ls, hb);
-            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, ls, hb);
+            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, rs, hb);
+            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, rs, hb);
             a0 = sp[kk + 4];
             a1 = sp[kk + 5];
-            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, ls, hb);
-            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, ls, hb);
+            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, rs, hb);
+            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, rs, hb);
             kk += 4;
         } while (ke - kk >= 4);
     }
-    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, ls, hb);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, rs, hb);
 }
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
 template <int R, bool SHARE_P>
 __device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ sp, int kk, const int ke,
                                                    const double (&invP)[R], const double (&cc)[R], const int n_phi,
-                                                   const uint32_t ls, const uint32_t (&hb)[(R + 1) / 2]) {
+                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2]) {
     for (; kk < ke; ++kk) {
         const double2 p = sp[kk];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
-            red_add_u32(((uint32_t)j << ls) + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
+            red_add_u32((uint32_t)j * rs + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
         }
     }
 }
 
-// S4, first half: close magnitude bin `seg_i` -- read and clear this thread's column of the phase histogram, add it to
-// the phase marginal, accumulate sum_j L(n_ij).  One phase bin j, all R trials.
+// S4, first half: close magnitude bin `seg_i`.  fetch_word reads and clears this thread's counter word of phase bin j
+// (two 16-bit counts, trials 2*w2 and 2*w2+1); close_word adds it to the phase marginal and accumulates sum L(n_ij).
+__device__ __forceinline__ uint32_t fetch_word(const int j, const int n_phi, const uint32_t rs, const uint32_t hbw) {
+    uint32_t w = exch0_u32(hbw + (uint32_t)j * rs);
+    if (j == 0) w += exch0_u32(hbw + (uint32_t)n_phi * rs);  // phase bin 0 takes over the overflow row
+    return w;
+}
+
 template <int R, bool DUMP, bool BIG>
-__device__ __forceinline__ void close_bin(const int j, const bool fold_overflow, const int n_phi, const uint32_t ls,
-                                          const uint32_t (&hb)[(R + 1) / 2], uint32_t (&mg)[(R + 1) / 2],
-                                          int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
-                                          const int lc, const int64_t s0, const bool (&valid)[R], const int seg_i) {
-    constexpr int RW = (R + 1) / 2;
-#pragma unroll
-    for (int w2 = 0; w2 < RW; ++w2) {
-        uint32_t w = exch0_u32(hb[w2] + ((uint32_t)j << ls));
-        if (fold_overflow) w += exch0_u32(hb[w2] + ((uint32_t)n_phi << ls));  // j == 0 takes over the overflow row
-        mg[w2] += w;
-        const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-        S2[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
-        if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
-        if (DUMP) {
-            if (valid[2 * w2])
-                prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
-            if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
-                prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * prm.n_m + seg_i] = c1;
-        }
+__device__ __forceinline__ void close_word(const uint32_t w, const int j, const int w2, const int n_phi,
+                                           int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
+                                           const int lc, const int64_t s0, const bool (&valid)[R], const int seg_i) {
+    const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
+    S2[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
+    if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
+    if (DUMP) {
+        if (valid[2 * w2])
+            prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
+        if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
+            prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * prm.n_m + seg_i] = c1;
     }
 }
 
-// All phase bins of magnitude bin seg_i.  MG: phase marginal, registers (NPHI > 0) or shared memory (NPHI == 0).
-template <int NPHI, int R, bool DUMP, bool BIG>
-__device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t ls, const uint32_t marg_off,
+// All phase bins of magnitude bin seg_i.  The phase marginal is a register array (REGM, compile-time n_phi) or a second
+// set of counter rows in shared memory updated with one RED per word (no registers, so more threads fit per SM).
+// With a compile-time n_phi the read-and-clear atomics of kCloseGroup phase bins are issued back to back before
+// their results are used, so their latency overlaps.
+template <int NPHI, bool REGM, int R, bool DUMP, bool BIG>
+__device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off,
                                               const uint32_t (&hb)[(R + 1) / 2],
-                                              uint32_t (&mg)[NPHI > 0 ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
+                                              uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
                                               const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
                                               const int64_t s0, const bool (&valid)[R], const int seg_i) {
     constexpr int RW = (R + 1) / 2;
     if (NPHI > 0) {
+        constexpr int NP = NPHI > 0 ? NPHI : 1;
+        constexpr int G = NP % kCloseGroup == 0 ? kCloseGroup : 1;
 #pragma unroll
-        for (int j = 0; j < (NPHI > 0 ? NPHI : 1); ++j)
-            close_bin<R, DUMP, BIG>(j, j == 0, n_phi, ls, hb, mg[j], S2, sL, prm, lc, s0, valid, seg_i);
+        for (int j0 = 0; j0 < NP; j0 += G) {
+            uint32_t w[G][RW];
+#pragma unroll
+            for (int jj = 0; jj < G; ++jj)
+#pragma unroll
+                for (int w2 = 0; w2 < RW; ++w2) w[jj][w2] = fetch_word(j0 + jj, n_phi, rs, hb[w2]);
+#pragma unroll
+            for (int jj = 0; jj < G; ++jj)
+#pragma unroll
+                for (int w2 = 0; w2 < RW; ++w2) {
+                    if (REGM) mg[REGM ? j0 + jj : 0][w2] += w[jj][w2];
+                    else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, w[jj][w2]);
+                    close_word<R, DUMP, BIG>(w[jj][w2], j0 + jj, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                }
+        }
     } else {
         for (int j = 0; j < n_phi; ++j) {
-            uint32_t m2[RW];
 #pragma unroll
-            for (int w2 = 0; w2 < RW; ++w2) m2[w2] = lds_u32(hb[w2] + marg_off + ((uint32_t)j << ls));
-            close_bin<R, DUMP, BIG>(j, j == 0, n_phi, ls, hb, m2, S2, sL, prm, lc, s0, valid, seg_i);
-#pragma unroll
-            for (int w2 = 0; w2 < RW; ++w2) sts_u32(hb[w2] + marg_off + ((uint32_t)j << ls), m2[w2]);
+            for (int w2 = 0; w2 < RW; ++w2) {
+                const uint32_t w = fetch_word(j, n_phi, rs, hb[w2]);
+                red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, w);
+                close_word<R, DUMP, BIG>(w, j, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+            }
         }
     }
 }
 
-// NPHI > 0: compile-time n_phi, 512 threads, phase marginal in registers.  NPHI == 0: any n_phi <= 64, threads per CTA
-// = 1 << prm.log2nt, marginal in shared memory.  R = trials per thread.  SHARE_P: the R trials of a thread share one
-// period (n_pdot % R == 0).  DUMP: test mode, trials come from a list and the count tables are written out.
-template <int NPHI, int R, bool SHARE_P, bool DUMP>
-__global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
+// NPHI > 0: compile-time n_phi (unrolled S4); NPHI == 0: any n_phi <= 64.  REGM: phase marginal in registers, exactly
+// 512 threads per CTA; otherwise the marginal is a second set of counter rows in shared memory, threads per CTA =
+// prm.nt (any multiple of 32 up to 640), which leaves registers for a fifth warp per sub-partition when the shared
+// memory allows it.  R = trials per thread.  SHARE_P: the R trials of a thread share one period (n_pdot % R == 0).
+// DUMP: test mode, trials come from a list and the count tables are written out.
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP>
+__global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchParams prm) {
+    static_assert(!REGM || NPHI > 0, "register marginals need a compile-time n_phi");
     constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
-    constexpr bool REGM = NPHI > 0;
     constexpr int NPHI_REG = REGM ? NPHI : 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int NT = blockDim.x, NW = NT >> 5;
+    const int NT = REGM ? 512 : (int)blockDim.x, NW = NT >> 5;
     const int tid = threadIdx.x, lane = tid & 31;
-    const int n_phi = REGM ? NPHI : prm.n_phi, n_m = prm.n_m;
-    const uint32_t ls = (uint32_t)(REGM ? kFastLog2NT : prm.log2nt) + 2u;  // log2(bytes between phase bins)
+    const int n_phi = NPHI > 0 ? NPHI : prm.n_phi, n_m = prm.n_m;
+    const uint32_t rs = (uint32_t)NT * 4u;  // bytes between the counter rows of consecutive phase bins
 
     // shared-memory carve-up: the L table first (compile-time offset, so lookups are LDS.64 [c*8 + imm]), points last
     int64_t *sL = reinterpret_cast<int64_t *>(smem_raw);                         // [kLtabSmem]
     uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);               // [2]
     int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
     uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 4);   // [RW][n_phi + 1][NT], 16-byte aligned
-    const uint32_t plane = (uint32_t)(n_phi + 1) * (uint32_t)NT * 4u;            // bytes per counter-word plane
-    const uint32_t marg_off = (uint32_t)RW * plane;                              // NPHI == 0: marg follows hist
-    double2 *spts = reinterpret_cast<double2 *>(reinterpret_cast<unsigned char *>(hist) +
-                                                (size_t)(REGM ? RW : 2 * RW) * plane);  // [cap_points]
+    const uint32_t plane = (uint32_t)(n_phi + 1) * rs;                           // bytes per counter-word plane
+    // shared-memory marginal (!REGM): RW planes of n_phi rows after the histogram; word (w2, j) of this thread is at
+    // hb[w2] + marg_off + (j - w2) * rs
+    const uint32_t marg_off = (uint32_t)RW * plane;
+    const uint32_t hist_words = (uint32_t)(REGM ? RW * (n_phi + 1) : RW * (2 * n_phi + 1)) * (uint32_t)NT;
+    double2 *spts = reinterpret_cast<double2 *>(hist + hist_words);              // [cap_points + 2]
 
     const int lc = blockIdx.x / prm.jobs_per_lc;
     const int job = blockIdx.x % prm.jobs_per_lc;
@@ -446,7 +457,7 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
     };
 
     // ---- prologue: zero histograms, stage table / segments, start the point loads
-    for (int i = tid; i < (REGM ? RW : 2 * RW) * (n_phi + 1) * NT; i += NT) hist[i] = 0u;
+    for (uint32_t i = tid; i < hist_words; i += NT) hist[i] = 0u;
     for (int i = tid; i < kLtabSmem; i += NT) sL[i] = i < prm.ltab_n ? prm.ltab[i] : 0;
     for (int i = tid; i <= n_m; i += NT) sseg[i] = prm.seg[(int64_t)lc * (n_m + 1) + i];
     if (tid == 0) {
@@ -479,7 +490,8 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
     // sums do not depend on the order of the bins.  Streamed light curves are processed in storage order.
     int rot = 0;
     if (single && n_m > 1) {
-        const int target = (int)(((int64_t)N * ((tid >> 7) & 3)) >> 2);
+        const int groups = (NW + 3) >> 2;
+        const int target = (int)((int64_t)N * (tid >> 7) / groups);
         while (rot + 1 < n_m && sseg[rot + 1] <= target) ++rot;
     }
     int g = 0;  // position in this CTA's chunk sequence (streamed mode)
@@ -529,19 +541,19 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, ls, hb);
-                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, ls, hb);
+                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb);
+                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb);
                     } else {
-                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, ls, hb);
+                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb);
                     }
                 }
                 if (b1 > k_end) break;  // the bin continues in the next buffer
                 // ---------------- S4: the bin is complete; a cell holds at most b1 - b0 points
                 if (b1 > b0) {
                     if (b1 - b0 < kLtabSmem)
-                        close_mag_bin<NPHI, R, DUMP, false>(n_phi, ls, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        close_mag_bin<NPHI, REGM, R, DUMP, false>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                     else
-                        close_mag_bin<NPHI, R, DUMP, true>(n_phi, ls, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        close_mag_bin<NPHI, REGM, R, DUMP, true>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                 }
                 ++seg_s;
             }
@@ -572,7 +584,7 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
                 } else {
                     for (int j = 0; j < n_phi; ++j)
 #pragma unroll
-                        for (int w2 = 0; w2 < RW; ++w2) add_marg(exch0_u32(hb[w2] + marg_off + ((uint32_t)j << ls)), w2, big);
+                        for (int w2 = 0; w2 < RW; ++w2) add_marg(exch0_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs), w2, big);
                 }
             };
             if (N < kLtabSmem) marg_pass(FalseT{}); else marg_pass(TrueT{});
@@ -614,7 +626,7 @@ __global__ void __launch_bounds__(512, 1) k_search(const SearchParams prm) {
     if (!DUMP && prm.top_k > 0) {
         const int K = prm.top_k;
         __syncthreads();  // every issued TMA load has been consumed: the point buffer is idle, reuse it as scratch
-        int64_t *scr = reinterpret_cast<int64_t *>(spts);  // 16 * NW * K <= 8 KB <= cap_points * 16 (cap >= 512)
+        int64_t *scr = reinterpret_cast<int64_t *>(spts);  // 16 * NW * K <= 10 KB <= cap_points * 16 (cap >= kMinPoints)
         if (lane < K) {
             scr[2 * ((tid >> 5) * K + lane)] = top.S;
             scr[2 * ((tid >> 5) * K + lane) + 1] = top.q;
@@ -710,43 +722,66 @@ struct Plan {
     int R;             // trials per thread
     bool share_p;      // the R trials of a thread share one period
     int nphi_t;        // compile-time n_phi of the kernel (15, 20, 30) or 0 = generic
-    int log2nt;        // threads per CTA = 1 << log2nt
+    bool regm;         // phase marginal in registers (512 threads) instead of shared memory
+    int nt;            // threads per CTA (multiple of 32)
     int cap_points;    // shared-memory point buffer capacity
     size_t smem;       // dynamic shared memory per CTA
     int64_t tiles_per_lc;
     int jobs_per_lc;
 };
 
+constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-marginal kernels (<= 102 registers)
+constexpr int kMinPoints = 640;           // smallest point buffer; also the top-k merge scratch (16 B x 20 warps x 32)
+
 size_t search_smem_fixed() {
     return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4);
 }
-size_t search_smem_planes(int n_phi, int R, bool regm, int nt) {
-    const int RW = (R + 1) / 2;
-    return (size_t)(regm ? RW : 2 * RW) * (size_t)(n_phi + 1) * (size_t)nt * sizeof(uint32_t);
+// counter rows of one thread: histogram (n_phi + 1 rows, the last one catches RN(x * n_phi) == n_phi * (floor(x) + 1)),
+// plus n_phi marginal rows when the marginal is not in registers; RW words each
+size_t search_smem_per_thread(int n_phi, int R, bool regm) {
+    return (size_t)((R + 1) / 2) * (size_t)(regm ? n_phi + 1 : 2 * n_phi + 1) * sizeof(uint32_t);
 }
 
-Plan make_plan(int32_t n_lc, int64_t n_trials, int64_t n_pdot, int n_phi, bool dump) {
+Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_pdot, int n_phi, bool dump) {
     Plan p;
     if (dump) { p.R = 2; p.share_p = false; }
     else if (n_pdot % 4 == 0) { p.R = 4; p.share_p = true; }
     else if (n_pdot % 2 == 0) { p.R = 2; p.share_p = true; }
     else { p.R = 4; p.share_p = false; }
-    const size_t fixed = search_smem_fixed();
-    const size_t min_pts = (512 + 2) * sizeof(double2);  // also the top-k merge scratch
-    p.nphi_t = 0;
-    if (!dump && (n_phi == 15 || n_phi == 20 || n_phi == 30) &&
-        fixed + search_smem_planes(n_phi, p.R, true, 1 << kFastLog2NT) + min_pts <= (size_t)kSmemLimit)
-        p.nphi_t = n_phi;
-    p.log2nt = kFastLog2NT;
-    if (p.nphi_t == 0)
-        while (p.log2nt > 5 && fixed + search_smem_planes(n_phi, p.R, false, 1 << p.log2nt) + min_pts > (size_t)kSmemLimit) --p.log2nt;
-    const size_t planes = search_smem_planes(n_phi, p.R, p.nphi_t != 0, 1 << p.log2nt);
-    int64_t cap = ((int64_t)kSmemLimit - (int64_t)fixed - (int64_t)planes) / (int64_t)sizeof(double2) - 2;
+    const int64_t avail = (int64_t)kSmemLimit - (int64_t)search_smem_fixed();
+    const bool templ = !dump && (n_phi == 15 || n_phi == 20 || n_phi == 30);
+    // point buffer wanted: the average light curve plus a quarter (the per-LC lengths live on the device; a longer
+    // light curve is streamed through the buffer in two halves instead of staying resident)
+    const int64_t avg = n_lc > 0 ? (total_points + n_lc - 1) / n_lc : 0;
+    int64_t want_pts = (avg + avg / 4 + 15) / 8 * 8;
+    if (want_pts < kMinPoints) want_pts = kMinPoints;
+    if (want_pts > 8192) want_pts = 8192;
+    auto threads_beside = [&](int64_t pts, bool regm) {
+        int64_t nt = (avail - (pts + 2) * (int64_t)sizeof(double2)) / (int64_t)search_smem_per_thread(n_phi, p.R, regm);
+        return nt < 0 ? 0 : nt / 32 * 32;
+    };
+    int64_t nt_s = threads_beside(want_pts, false);
+    if (nt_s > kMaxThreadsSmemMarg) nt_s = kMaxThreadsSmemMarg;
+    const bool regm_fits = templ && threads_beside(kMinPoints, true) >= 512;
+    // measured on C3: 512 threads with register marginals beat 608 threads with shared-memory
+    // marginals (83.7 vs 86.8 ms), so the register variant is taken whenever it fits
+    if (regm_fits) {
+        p.regm = true;
+        p.nt = 512;
+    } else {
+        p.regm = false;
+        if (nt_s < 32) nt_s = threads_beside(kMinPoints, false);
+        if (nt_s > kMaxThreadsSmemMarg) nt_s = kMaxThreadsSmemMarg;
+        p.nt = (int)nt_s;  // >= 32: 64 x 64 bins with R = 4 leave room for 192 threads
+    }
+    p.nphi_t = templ ? n_phi : 0;
+    const int64_t planes = (int64_t)search_smem_per_thread(n_phi, p.R, p.regm) * p.nt;
+    int64_t cap = (avail - planes) / (int64_t)sizeof(double2) - 2;  // - 2: read-ahead slack of the hot loop
     cap = cap / 8 * 8;
     if (cap > 8192) cap = 8192;  // 128 KB of points; longer light curves are streamed
     p.cap_points = (int)cap;
-    p.smem = (size_t)(cap + 2) * sizeof(double2) + fixed + planes;  // + 2: read-ahead slack of the hot loop
-    const int64_t tile = (int64_t)(1 << p.log2nt) * p.R;
+    p.smem = (size_t)(cap + 2) * sizeof(double2) + search_smem_fixed() + (size_t)planes;
+    const int64_t tile = (int64_t)p.nt * p.R;
     p.tiles_per_lc = n_trials > 0 ? (n_trials + tile - 1) / tile : 0;
     // ~16 CTAs per SM overall for dynamic balance, at least one tile per job
     int64_t want = (148LL * 16 + (n_lc > 0 ? n_lc : 1) - 1) / (n_lc > 0 ? n_lc : 1);
@@ -771,7 +806,7 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     int64_t tn = total_points < GCE_CE_MAX_POINTS ? total_points : GCE_CE_MAX_POINTS;
     L.ltab_n = (int)tn + 1;
     L.ltab = o; o = align_up(o + sizeof(int64_t) * (size_t)L.ltab_n, 256);
-    const Plan p = make_plan(n_lc, n_trials, n_pdot, prm->n_phase_bins, dump);
+    const Plan p = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins, dump);
     const size_t parts = (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc * (size_t)(prm->top_k > 0 ? prm->top_k : 1);
     L.part_S = o; o = align_up(o + sizeof(int64_t) * parts, 256);
     L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
@@ -815,32 +850,32 @@ int cuda_fail(cudaError_t e) {
     return GCE_CE_ERR_CUDA;
 }
 
-template <int NPHI, int R, bool SHARE_P, bool DUMP>
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP>
 int launch_search(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
-    auto kern = k_search<NPHI, R, SHARE_P, DUMP>;
+    auto kern = k_search<NPHI, REGM, R, SHARE_P, DUMP>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem);
     if (e != cudaSuccess) return cuda_fail(e);
     const unsigned grid = (unsigned)((int64_t)n_lc * plan.jobs_per_lc);
-    kern<<<grid, 1 << plan.log2nt, plan.smem, st>>>(sp);
+    kern<<<grid, plan.nt, plan.smem, st>>>(sp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return GCE_CE_OK;
 }
 
-template <int NPHI>
+template <int NPHI, bool REGM>
 int launch_search_variant(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
-    if (plan.share_p && plan.R == 4) return launch_search<NPHI, 4, true, false>(sp, plan, n_lc, st);
-    if (plan.share_p && plan.R == 2) return launch_search<NPHI, 2, true, false>(sp, plan, n_lc, st);
-    return launch_search<NPHI, 4, false, false>(sp, plan, n_lc, st);
+    if (plan.share_p && plan.R == 4) return launch_search<NPHI, REGM, 4, true, false>(sp, plan, n_lc, st);
+    if (plan.share_p && plan.R == 2) return launch_search<NPHI, REGM, 2, true, false>(sp, plan, n_lc, st);
+    return launch_search<NPHI, REGM, 4, false, false>(sp, plan, n_lc, st);
 }
 
 int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t n_lc, cudaStream_t st) {
-    if (dump) return launch_search<0, 2, false, true>(sp, plan, n_lc, st);
+    if (dump) return launch_search<0, false, 2, false, true>(sp, plan, n_lc, st);
     switch (plan.nphi_t) {
-        case 15: return launch_search_variant<15>(sp, plan, n_lc, st);
-        case 20: return launch_search_variant<20>(sp, plan, n_lc, st);
-        case 30: return launch_search_variant<30>(sp, plan, n_lc, st);
-        default: return launch_search_variant<0>(sp, plan, n_lc, st);
+        case 15: return plan.regm ? launch_search_variant<15, true>(sp, plan, n_lc, st) : launch_search_variant<15, false>(sp, plan, n_lc, st);
+        case 20: return plan.regm ? launch_search_variant<20, true>(sp, plan, n_lc, st) : launch_search_variant<20, false>(sp, plan, n_lc, st);
+        case 30: return plan.regm ? launch_search_variant<30, true>(sp, plan, n_lc, st) : launch_search_variant<30, false>(sp, plan, n_lc, st);
+        default: return launch_search_variant<0, false>(sp, plan, n_lc, st);
     }
 }
 
@@ -922,7 +957,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
 
-    const Plan plan = make_plan(n_lc, n_trials, dump ? 1 : n_pdot, prm->n_phase_bins, dump);
+    const Plan plan = make_plan(n_lc, total_points, n_trials, dump ? 1 : n_pdot, prm->n_phase_bins, dump);
     SearchParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.pts = pts; sp.seg = seg; sp.info = info; sp.lc_offsets = lc_offsets; sp.ltab = ltab;
@@ -930,7 +965,6 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.n_p = n_p; sp.n_pdot = n_pdot; sp.n_trials = n_trials;
     sp.jobs_per_lc = plan.jobs_per_lc;
     sp.tiles_per_lc = plan.tiles_per_lc;
-    sp.log2nt = plan.log2nt;
     sp.cap_points = plan.cap_points;
     sp.n_phi = prm->n_phase_bins; sp.n_m = prm->n_mag_bins;
     sp.ltab_n = L.ltab_n;
