@@ -43,6 +43,10 @@ METRIC = "CE point-folds/sec"
 UNIT = "point-folds/s"
 FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (probe-measured)
 N_SM = 148
+# DRAM traffic of one k_search launch from the committed ncu --set full capture (profiles/r1_k_search_C3_full.md):
+# 17.1 MB read + 773.2 MB written; the algorithmic output is the 819.2 MB fp32 cube (part of it is still in L2 at
+# kernel end).  Only workloads that were captured have an entry.
+NCU_DRAM_BYTES_PER_LAUNCH = {"C3": 17.1e6 + 773.2e6}
 
 
 def load_peaks():
@@ -250,12 +254,8 @@ def run_ours(args):
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     step_ms = [s.elapsed_time(e) for s, e in zip(s_ev, e_ev)]
     tot_ms = float(sum(step_ms))
-    t = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
-    pf = torch.tensor([float(w.point_folds)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(pf, op=dist.ReduceOp.SUM)
-    tot_ms_max, pf_all = float(t.item()), float(pf.item())
+    from paper_2006_06866_b200 import sharding
+    tot_ms_max, pf_all = sharding.reduce_timing(tot_ms, float(w.point_folds), dist if world > 1 else None, dev)
     value = pf_all * args.steps / (tot_ms_max * 1e-3)
 
     # ---- end to end through the host entry point: pinned host buffers, H2D + D2H + allocation inside the timing
@@ -294,7 +294,10 @@ def run_ours(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = FP64_LANES_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9      # at the maximum SM clock (strictest denominator)
     roof = {"bound": "alu", "pipe": "fp64", "kernel": "k_search", "achieved": achieved, "peak": peak,
-            "unit": "G FP64 lane-ops/s", "frac": achieved / peak, "traffic": None,
+            "unit": "G FP64 lane-ops/s", "frac": achieved / peak,
+            "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if not args.quick else None,
+            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_search launch, ncu --set full "
+                              "(profiles/r1_k_search_C3_full.md); bytes per launch",
             "peak_source": f"64 FP64 lanes/SM/clk x 148 SMs x {sm_max:.0f} MHz (max SM clock, {peaks_src} MEASURED_PEAKS.json; "
                            "per-SM rate probe-measured, DESIGN.md section 7)",
             "algorithmic_ops_per_point_fold": algorithmic_fp64_ops_per_pointfold(w),
