@@ -75,8 +75,10 @@ int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int6
  *   out_best_idx     NULL (iff top_k == 0), or int64[n_lc][top_k]: flat q of the k smallest CE, ascending by
  *                    (CE, q); -1 where fewer than k trials exist or N = 0
  *   out_best_ce      NULL, or float[n_lc][top_k] matching out_best_idx (NaN where idx = -1)
- *   out_stats        NULL, or double[n_lc][4] = {mean CE, population std, min CE, rho = (mean-min)/std}
- *                    over all trials of the light curve (Eq. 5)
+ *   out_stats        NULL (iff want_stats == 0), or double[n_lc][4] = {mean CE, population std, min CE,
+ *                    rho = (mean-min)/std} over all trials of the light curve (Eq. 5); exact
+ *                    integer partial sums inside, so the values do not depend on the CTA split; std = 0 exactly
+ *                    and rho = NaN when every trial has the same CE; all NaN for N = 0
  * At least one of out_ce / out_best_idx / out_stats must be non-NULL.
  */
 int gce_ce_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,

@@ -43,6 +43,8 @@ constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(
 constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
 constexpr int64_t kInfS = INT64_MAX;
 constexpr int kSmemLimit = 227 * 1024;
+constexpr int kStatWords = 8;     // partial Eq. 5 sums: n, sum d (i128), sum d^2 (u192), min S, pad; d = S - K
+constexpr int kMaxWarps = 20;     // warps per CTA of the largest variant (640 threads)
 constexpr int kCloseGroup = 5;    // phase bins whose read-and-clear atomics are in flight together in S4
 
 struct FalseT { static constexpr bool value = false; };
@@ -52,6 +54,7 @@ struct LcInfo {
     int32_t n;
     int32_t pad;
     double dt_max;
+    int64_t K;  // N * H(m) in 2^-42 fixed point = L(N) - sum_i L(points in magnitude bin i): CE <= H(m), pivot of the Eq. 5 sums
 };
 
 struct SearchParams {
@@ -73,6 +76,7 @@ struct SearchParams {
     int32_t ce_fp64;
     void *out_ce;              // cube or NULL
     int64_t *part_S, *part_q;  // [n_lc][jobs_per_lc][top_k]
+    uint64_t *part_stats;      // [n_lc][jobs_per_lc][kStatWords] partial Eq. 5 sums, or NULL
     uint32_t *out_counts;      // DUMP only
     double *out_ce_at;         // DUMP only
 };
@@ -143,6 +147,35 @@ struct WarpTopK {
     }
 };
 
+// ---- Eq. 5 statistics (NEXT item N1): exact integer partial sums of d = S - K over trials, S = N*CE*2^42.
+// Word layout (kStatWords u64): [0] n, [1..2] sum d (two's-complement i128), [3..5] sum d^2 (u192), [6] min S, [7] max S.
+typedef unsigned __int128 u128_t;
+__device__ __forceinline__ u128_t shfl_xor_u128(u128_t v, int o) {
+    uint64_t lo = (uint64_t)v, hi = (uint64_t)(v >> 64);
+    lo = __shfl_xor_sync(0xffffffffu, lo, o);
+    hi = __shfl_xor_sync(0xffffffffu, hi, o);
+    return ((u128_t)hi << 64) | lo;
+}
+__device__ __forceinline__ void stat_init(uint64_t *st) {
+    st[0] = st[1] = st[2] = st[3] = st[4] = st[5] = 0;
+    st[6] = (uint64_t)kInfS;
+    st[7] = (uint64_t)INT64_MIN;
+}
+// st += (n, a, b, mn, mx); a is an i128 passed as its two's-complement bits, b < 2^128
+__device__ __forceinline__ void stat_add(uint64_t *st, uint64_t n, u128_t a, u128_t b, uint64_t b_hi, int64_t mn, int64_t mx) {
+    st[0] += n;
+    const u128_t A = (((u128_t)st[2] << 64) | st[1]) + a;
+    st[1] = (uint64_t)A; st[2] = (uint64_t)(A >> 64);
+    const u128_t B = (((u128_t)st[4] << 64) | st[3]) + b;
+    st[3] = (uint64_t)B; st[4] = (uint64_t)(B >> 64);
+    st[5] += b_hi + (B < b ? 1u : 0u);
+    if (mn < (int64_t)st[6]) st[6] = (uint64_t)mn;
+    if (mx > (int64_t)st[7]) st[7] = (uint64_t)mx;
+}
+__device__ __forceinline__ void stat_merge(uint64_t *st, const uint64_t *o) {
+    stat_add(st, o[0], ((u128_t)o[2] << 64) | o[1], ((u128_t)o[4] << 64) | o[3], o[5], (int64_t)o[6], (int64_t)o[7]);
+}
+
 // S1 magnitude bin: min(floor(((m - m_lo) / r) * n_m), n_m - 1); r == 0 -> 0.
 __device__ __forceinline__ int mag_bin(double m, double m_lo, double r, int n_m) {
     if (r == 0.0) return 0;
@@ -203,7 +236,7 @@ __device__ __forceinline__ MinMax3 block_minmax(MinMax3 v, MinMax3 *sh) {
 __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ times, const double *__restrict__ mags,
                                                     const int64_t *__restrict__ lc_offsets, int n_m,
                                                     double2 *__restrict__ pts, int32_t *__restrict__ seg,
-                                                    LcInfo *__restrict__ info) {
+                                                    LcInfo *__restrict__ info, const int64_t *__restrict__ ltab) {
     __shared__ MinMax3 sh_red[8];
     __shared__ int sh_cnt[GCE_CE_MAX_BINS + 1];
     __shared__ int sh_cur[GCE_CE_MAX_BINS];
@@ -229,12 +262,15 @@ __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ t
     __syncthreads();
     if (threadIdx.x == 0) {
         int acc = 0;
+        int64_t K = ltab[n];
         for (int i = 0; i < n_m; ++i) {
             const int c = sh_cnt[i];
             seg[(int64_t)lc * (n_m + 1) + i] = acc;
             sh_cur[i] = acc;
             acc += c;
+            K -= ltab[c];
         }
+        info[lc].K = K;
         seg[(int64_t)lc * (n_m + 1) + n_m] = acc;
         info[lc].n = n;
         info[lc].pad = 0;
@@ -426,7 +462,8 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     int64_t *sL = reinterpret_cast<int64_t *>(smem_raw);                         // [kLtabSmem]
     uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);               // [2]
     int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
-    uint32_t *hist = reinterpret_cast<uint32_t *>(sseg + GCE_CE_MAX_BINS + 4);   // [RW][n_phi + 1][NT], 16-byte aligned
+    uint64_t *sstat = reinterpret_cast<uint64_t *>(sseg + GCE_CE_MAX_BINS + 4);  // [kMaxWarps][kStatWords]
+    uint32_t *hist = reinterpret_cast<uint32_t *>(sstat + kMaxWarps * kStatWords); // [RW][n_phi + 1][NT], 16-byte aligned
     const uint32_t plane = (uint32_t)(n_phi + 1) * rs;                           // bytes per counter-word plane
     // shared-memory marginal (!REGM): RW planes of n_phi rows after the histogram; word (w2, j) of this thread is at
     // hb[w2] + marg_off + (j - w2) * rs
@@ -441,6 +478,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     const int n_tiles = (int)(tile_hi - tile_lo);
     const int N = prm.info[lc].n;
     const double dt_max = prm.info[lc].dt_max;
+    const int64_t K = prm.info[lc].K;
     const double2 *gpts = prm.pts + prm.lc_offsets[lc];
     const bool single = N <= prm.cap_points;            // the whole light curve stays resident for every tile
     const int CH = single ? N : prm.cap_points / 2;     // else: streamed through two half buffers, per tile
@@ -460,6 +498,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     for (uint32_t i = tid; i < hist_words; i += NT) hist[i] = 0u;
     for (int i = tid; i < kLtabSmem; i += NT) sL[i] = i < prm.ltab_n ? prm.ltab[i] : 0;
     for (int i = tid; i <= n_m; i += NT) sseg[i] = prm.seg[(int64_t)lc * (n_m + 1) + i];
+    if (tid < NW) stat_init(sstat + tid * kStatWords);
     if (tid == 0) {
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
@@ -619,6 +658,44 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
 #pragma unroll
                 for (int r = 0; r < R; ++r) top.offer((valid[r] && N > 0) ? S[r] : kInfS, (valid[r] && N > 0) ? qv[r] : kInfS);
             }
+            if (prm.part_stats != nullptr && N > 0) {  // Eq. 5 partial sums of this tile, warp-reduced, exact integers
+                __int128 a = 0;
+                u128_t b = 0;
+                int64_t mn = kInfS, mx = INT64_MIN;
+                uint32_t cnt = 0;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (!valid[r]) continue;
+                    const int64_t d = S[r] - K;   // |d| < 2^60
+                    a += d;
+                    b += (u128_t)((__int128)d * d);
+                    mn = S[r] < mn ? S[r] : mn;
+                    mx = S[r] > mx ? S[r] : mx;
+                    ++cnt;
+                }
+                u128_t au = (u128_t)a;
+                for (int o = 16; o > 0; o >>= 1) {
+                    au += shfl_xor_u128(au, o);
+                    b += shfl_xor_u128(b, o);            // <= 32 * R * 2^120 < 2^128
+                    const int64_t m2 = __shfl_xor_sync(0xffffffffu, mn, o), m3 = __shfl_xor_sync(0xffffffffu, mx, o);
+                    mn = m2 < mn ? m2 : mn;
+                    mx = m3 > mx ? m3 : mx;
+                    cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+                }
+                if (lane == 0) stat_add(sstat + (tid >> 5) * kStatWords, cnt, au, b, 0, mn, mx);
+            }
+        }
+    }
+
+    // ---------------- per-CTA Eq. 5 partial sums -> part_stats[lc][job]
+    if (!DUMP && prm.part_stats != nullptr) {
+        __syncthreads();
+        if (tid == 0) {
+            uint64_t tot[kStatWords];
+            stat_init(tot);
+            for (int w = 0; w < NW; ++w) stat_merge(tot, sstat + w * kStatWords);
+            uint64_t *o = prm.part_stats + ((int64_t)lc * prm.jobs_per_lc + job) * kStatWords;
+            for (int i = 0; i < kStatWords; ++i) o[i] = tot[i];
         }
     }
 
@@ -669,6 +746,41 @@ __global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ p
         out_idx[(int64_t)lc * K + lane] = have ? top.q : -1;
         if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)n)) : CUDART_NAN_F;
     }
+}
+
+// Eq. 5: one warp per light curve sums the per-CTA partials (exact integers, so the result does not
+// depend on how the trials were split over CTAs, batches or GPUs) and converts once to fp64:
+// out_stats[lc] = {mean CE, population std, min CE, rho = (mean - min) / std}.
+__device__ __forceinline__ double u128_to_double(u128_t v) {
+    return (double)(uint64_t)(v >> 64) * 18446744073709551616.0 + (double)(uint64_t)v;
+}
+__global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__ part, const LcInfo *__restrict__ info,
+                                                    int jobs_per_lc, double *__restrict__ out_stats) {
+    __shared__ uint64_t sh[32][kStatWords];
+    const int lc = blockIdx.x, lane = threadIdx.x;
+    uint64_t acc[kStatWords];
+    stat_init(acc);
+    for (int j = lane; j < jobs_per_lc; j += 32) stat_merge(acc, part + ((int64_t)lc * jobs_per_lc + j) * kStatWords);
+    for (int i = 0; i < kStatWords; ++i) sh[lane][i] = acc[i];
+    __syncwarp();
+    if (lane != 0) return;
+    for (int l = 1; l < 32; ++l) stat_merge(acc, sh[l]);
+    double *o = out_stats + (int64_t)lc * 4;
+    const int n_pts = info[lc].n;
+    if (acc[0] == 0 || n_pts <= 0) { o[0] = o[1] = o[2] = o[3] = CUDART_NAN; return; }
+    const double n = (double)acc[0];
+    const u128_t A = ((u128_t)acc[2] << 64) | acc[1];
+    const bool neg = (acc[2] >> 63) != 0;
+    const double sum_d = neg ? -u128_to_double((u128_t)0 - A) : u128_to_double(A);
+    const double sum_d2 = (double)acc[5] * 3.4028236692093846e38 + u128_to_double(((u128_t)acc[4] << 64) | acc[3]);
+    const double scale = ldexp(1.0, -kLfixShift) / (double)n_pts;
+    const double mean_d = sum_d / n;
+    double var = sum_d2 / n - mean_d * mean_d;
+    if (var < 0.0 || acc[6] == acc[7]) var = 0.0;  // min == max: every trial has the same CE, the spread is exactly 0
+    const double mean = ((double)info[lc].K + mean_d) * scale;
+    const double sd = sqrt(var) * scale;
+    const double mn = (double)(int64_t)acc[6] * scale;
+    o[0] = mean; o[1] = sd; o[2] = mn; o[3] = (mean - mn) / sd;
 }
 
 // Test-only: bins of one light curve for one trial, caller's point order (same device functions as the path).
@@ -734,7 +846,8 @@ constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-m
 constexpr int kMinPoints = 640;           // smallest point buffer; also the top-k merge scratch (16 B x 20 warps x 32)
 
 size_t search_smem_fixed() {
-    return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4);
+    return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) +
+           sizeof(uint64_t) * kMaxWarps * kStatWords;
 }
 // counter rows of one thread: histogram (n_phi + 1 rows, the last one catches RN(x * n_phi) == n_phi * (floor(x) + 1)),
 // plus n_phi marginal rows when the marginal is not in registers; RW words each
@@ -793,7 +906,7 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
 }
 
 struct Layout {
-    size_t pts, seg, info, ltab, part_S, part_q, total;
+    size_t pts, seg, info, ltab, part_S, part_q, part_stats, total;
     int ltab_n;
 };
 
@@ -810,6 +923,8 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     const size_t parts = (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc * (size_t)(prm->top_k > 0 ? prm->top_k : 1);
     L.part_S = o; o = align_up(o + sizeof(int64_t) * parts, 256);
     L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
+    L.part_stats = o;
+    if (prm->want_stats) o = align_up(o + sizeof(uint64_t) * kStatWords * (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc, 256);
     L.total = o;
     return L;
 }
@@ -820,7 +935,8 @@ int check_params(const gce_ce_params *prm) {
     if (prm->n_mag_bins < 1 || prm->n_mag_bins > GCE_CE_MAX_BINS) return GCE_CE_ERR_RANGE;
     if (prm->top_k < 0 || prm->top_k > GCE_CE_MAX_TOPK) return GCE_CE_ERR_RANGE;
     if (prm->ce_fp64 != 0 && prm->ce_fp64 != 1) return GCE_CE_ERR_RANGE;
-    if (prm->want_stats != 0 || prm->overlap != 0) return GCE_CE_ERR_RANGE;  // NEXT items N1 / N2: not yet built
+    if (prm->want_stats != 0 && prm->want_stats != 1) return GCE_CE_ERR_RANGE;
+    if (prm->overlap != 0) return GCE_CE_ERR_RANGE;  // NEXT item N2: not yet built
     if (prm->reserved[0] != 0 || prm->reserved[1] != 0) return GCE_CE_ERR_RANGE;
     return GCE_CE_OK;
 }
@@ -901,7 +1017,7 @@ int gce_ce_last_cuda_error(void) { return g_last_cuda_error; }
 
 int gce_ce_launch_count(int32_t n_lc, const gce_ce_params *prm) {
     if (!prm || n_lc <= 0) return 0;
-    return 3 + (prm->top_k > 0 ? 1 : 0);  // preprocess, ltab, search, [merge]
+    return 3 + (prm->top_k > 0 ? 1 : 0) + (prm->want_stats ? 1 : 0);  // ltab, preprocess, search, [merge_topk], [merge_stats]
 }
 
 int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int64_t n_pdot, const gce_ce_params *prm,
@@ -917,7 +1033,7 @@ int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int6
 
 static int run_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                       int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                      const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                      const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce, double *out_stats,
                       const int64_t *trial_q, int64_t n_dump, uint32_t *out_counts, double *out_ce_at, void *workspace,
                       size_t workspace_bytes, void *stream) {
     const bool dump = out_counts != nullptr;
@@ -932,13 +1048,14 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     if (dump) {
         if (!trial_q || n_dump < 0) return GCE_CE_ERR_POINTER;
     } else {
-        if (!out_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+        if (!out_ce && !out_best_idx && !out_stats) return GCE_CE_ERR_POINTER;
+        if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
         if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
         if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
     }
     const int64_t n_trials = dump ? n_dump : n_p * n_pdot;
     gce_ce_params lay_prm = *prm;
-    if (dump) lay_prm.top_k = 0;
+    if (dump) { lay_prm.top_k = 0; lay_prm.want_stats = 0; }
     const Layout L = make_layout(total_points, n_lc, n_trials, dump ? 1 : n_pdot, &lay_prm, dump);
     if (workspace_bytes < L.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return GCE_CE_ERR_WORKSPACE;
     if (n_lc == 0) return GCE_CE_OK;
@@ -950,10 +1067,10 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     LcInfo *info = reinterpret_cast<LcInfo *>(ws + L.info);
     int64_t *ltab = reinterpret_cast<int64_t *>(ws + L.ltab);
 
-    k_preprocess<<<n_lc, 256, 0, st>>>(times, mags, lc_offsets, prm->n_mag_bins, pts, seg, info);
+    k_ltab<<<(L.ltab_n + 255) / 256, 256, 0, st>>>(ltab, L.ltab_n);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
-    k_ltab<<<(L.ltab_n + 255) / 256, 256, 0, st>>>(ltab, L.ltab_n);
+    k_preprocess<<<n_lc, 256, 0, st>>>(times, mags, lc_offsets, prm->n_mag_bins, pts, seg, info, ltab);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
 
@@ -973,6 +1090,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.out_ce = out_ce;
     sp.part_S = reinterpret_cast<int64_t *>(ws + L.part_S);
     sp.part_q = reinterpret_cast<int64_t *>(ws + L.part_q);
+    sp.part_stats = (!dump && prm->want_stats) ? reinterpret_cast<uint64_t *>(ws + L.part_stats) : nullptr;
     sp.out_counts = out_counts; sp.out_ce_at = out_ce_at;
 
     if (prm->ev_search_begin) {
@@ -993,6 +1111,11 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e);
     }
+    if (!dump && prm->want_stats) {
+        k_merge_stats<<<n_lc, 32, 0, st>>>(sp.part_stats, info, n_trials > 0 ? plan.jobs_per_lc : 0, out_stats);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
     return GCE_CE_OK;
 }
 
@@ -1000,9 +1123,8 @@ int gce_ce_search(const double *times, const double *mags, const int64_t *lc_off
                   int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
                   const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce, double *out_stats,
                   void *workspace, size_t workspace_bytes, void *stream) {
-    if (out_stats) return GCE_CE_ERR_RANGE;  // N1 not yet built
     return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, out_ce,
-                      out_best_idx, out_best_ce, nullptr, 0, nullptr, nullptr, workspace, workspace_bytes, stream);
+                      out_best_idx, out_best_ce, out_stats, nullptr, 0, nullptr, nullptr, workspace, workspace_bytes, stream);
 }
 
 int gce_ce_debug_histogram(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
@@ -1020,7 +1142,7 @@ int gce_ce_debug_histogram(const double *times, const double *mags, const int64_
         if (e != cudaSuccess) return cuda_fail(e);
     }
     return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, nullptr, nullptr,
-                      nullptr, trial_q, n_trials, out_counts, out_ce_at, workspace, workspace_bytes, stream);
+                      nullptr, nullptr, trial_q, n_trials, out_counts, out_ce_at, workspace, workspace_bytes, stream);
 }
 
 int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
@@ -1070,7 +1192,6 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
                        const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
                        const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
                        double *out_stats) {
-    if (out_stats) return GCE_CE_ERR_RANGE;
     int rc = check_params(prm);
     if (rc) return rc;
     if (!lc_offsets || n_lc < 0) return GCE_CE_ERR_POINTER;
@@ -1088,7 +1209,7 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
     cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
     if (e != cudaSuccess) return cuda_fail(e);
     void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
-    void *d_ce = nullptr, *d_idx = nullptr, *d_bce = nullptr;
+    void *d_ce = nullptr, *d_idx = nullptr, *d_bce = nullptr, *d_st = nullptr;
     auto dalloc = [&](void **p, size_t bytes) { return cudaMallocAsync(p, bytes ? bytes : 16, st); };
     rc = GCE_CE_OK;
     do {
@@ -1096,7 +1217,7 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
             (e = dalloc(&d_off, 8 * (size_t)(n_lc + 1))) || (e = dalloc(&d_p, 8 * (size_t)n_p)) ||
             (e = dalloc(&d_pd, 8 * (size_t)n_pdot)) || (e = dalloc(&d_ws, ws_bytes)) ||
             (e = dalloc(&d_ce, ce_bytes)) || (e = dalloc(&d_idx, 8 * (size_t)n_lc * k)) ||
-            (e = dalloc(&d_bce, 4 * (size_t)n_lc * k))) { rc = cuda_fail(e); break; }
+            (e = dalloc(&d_bce, 4 * (size_t)n_lc * k)) || (e = dalloc(&d_st, 32 * (size_t)n_lc))) { rc = cuda_fail(e); break; }
         if (total) {
             cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
             cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
@@ -1106,14 +1227,15 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
         cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st);
         rc = gce_ce_search((const double *)d_t, (const double *)d_m, (const int64_t *)d_off, n_lc, total,
                            (const double *)d_p, n_p, (const double *)d_pd, n_pdot, prm, out_ce ? d_ce : nullptr,
-                           out_best_idx ? (int64_t *)d_idx : nullptr, out_best_ce ? (float *)d_bce : nullptr, nullptr,
-                           d_ws, ws_bytes, st);
+                           out_best_idx ? (int64_t *)d_idx : nullptr, out_best_ce ? (float *)d_bce : nullptr,
+                           out_stats ? (double *)d_st : nullptr, d_ws, ws_bytes, st);
         if (rc) break;
         if (out_ce && ce_bytes) cudaMemcpyAsync(out_ce, d_ce, ce_bytes, cudaMemcpyDeviceToHost, st);
         if (out_best_idx && k) cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
         if (out_best_ce && k) cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
+        if (out_stats && n_lc) cudaMemcpyAsync(out_stats, d_st, 32 * (size_t)n_lc, cudaMemcpyDeviceToHost, st);
     } while (0);
-    void *frees[] = {d_t, d_m, d_off, d_p, d_pd, d_ws, d_ce, d_idx, d_bce};
+    void *frees[] = {d_t, d_m, d_off, d_p, d_pd, d_ws, d_ce, d_idx, d_bce, d_st};
     for (void *p : frees)
         if (p) cudaFreeAsync(p, st);
     e = cudaStreamSynchronize(st);

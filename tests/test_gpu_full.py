@@ -168,3 +168,92 @@ def test_long_light_curves_are_streamed(gce, oracle, n_obs, n_phi, n_m, n_pdot):
     torch.cuda.synchronize()
     refc = oracle.histogram(t_long, m_long, periods, pdots, n_phi, n_m, q.cpu().numpy())
     assert np.array_equal(counts[0].cpu().numpy().astype(np.int64), refc)
+
+
+# ------------------------------------------------------------------------------------------ N1: fused Eq. 5 statistics
+RTOL_STATS = 1e-9   # exact integer sums of N*CE*2^42, one fp64 conversion; the per-trial CE values
+                    # differ from the oracle's by <= 1e-12 relative, the variance subtraction amplifies that by mean^2/var
+
+
+def _stats_ref(oracle, ref_cube):
+    out = []
+    for row in ref_cube:
+        mu, sigma, rho = oracle.significance(row)
+        out.append((mu, sigma, float(np.min(row)) if row.size else np.nan, rho))
+    return np.array(out)
+
+
+@pytest.mark.parametrize("name,kw", [
+    ("C2", dict(n_lc=6, n_p=3000)),
+    ("C3", dict(n_lc=4, n_p=1500, n_pdot=64)),
+    ("C3", dict(n_lc=2, n_p=1111, n_pdot=7)),
+    ("C4", dict(n_lc=9, n_p=5000)),
+    ("C5", dict(n_lc=2, n_p=300, n_pdot=16)),
+])
+def test_fused_significance_matches_oracle(gce, oracle, name, kw):
+    """out_stats = {mean CE, population std, min CE, rho} (Eq. 5) against the oracle's Eq. 5 over the
+    oracle's cube; with and without the cube / top-k outputs (the no-cube mode is what N1 is for)."""
+    w = W.make(name, **kw)
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, w.n_phase_bins, w.n_mag_bins)
+    want = _stats_ref(oracle, ref.reshape(w.n_lc, -1))
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    args = (d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), w.n_phase_bins, w.n_mag_bins)
+    for top_k, cube in ((0, False), (3, False), (1, True)):
+        res = gce.search(*args, top_k=top_k, want_cube=cube, want_stats=True)
+        torch.cuda.synchronize()
+        got = res.stats.cpu().numpy()
+        np.testing.assert_allclose(got, want, rtol=RTOL_STATS, atol=1e-13)
+        if top_k:
+            assert np.allclose(got[:, 2], res.best_ce[:, 0].cpu().numpy().astype(np.float64), rtol=1e-6)
+
+
+def test_fused_significance_degenerate_and_split_invariance(gce, oracle):
+    """N = 0 -> NaN; constant CE (n_phi = 1, or all magnitudes equal) -> std exactly 0 and rho NaN like the oracle's 0/0;
+    the statistics do not depend on how the trials are split over CTAs (exact integer partial sums)."""
+    rng = np.random.default_rng(3)
+    lcs = [(np.zeros(0), np.zeros(0)), (np.sort(rng.uniform(0, 1e6, 400)), np.full(400, 3.0)),
+           (np.sort(rng.uniform(0, 1e6, 700)), rng.normal(size=700))]
+    times = np.concatenate([t for t, _ in lcs]); mags = np.concatenate([m for _, m in lcs])
+    offs = np.cumsum([0] + [t.size for t, _ in lcs]).astype(np.int64)
+    periods = 1.0 / np.linspace(1 / 5000.0, 1 / 50.0, 4099)
+    pdots = np.linspace(-1e-9, 0, 3)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(times), d(mags), d(offs), d(periods), d(pdots), 20, 10, top_k=0, want_cube=True, ce_fp64=True,
+                     want_stats=True)
+    torch.cuda.synchronize()
+    st = res.stats.cpu().numpy()
+    assert np.all(np.isnan(st[0]))
+    assert st[1, 0] == 0.0 and st[1, 1] == 0.0 and st[1, 2] == 0.0 and np.isnan(st[1, 3])
+    cube = res.ce.cpu().numpy().reshape(3, -1)
+    assert st[2, 0] == pytest.approx(cube[2].mean(), rel=1e-12)
+    assert st[2, 1] == pytest.approx(cube[2].std(), rel=1e-9)
+    assert st[2, 2] == cube[2].min()
+    # n_phi = 1: CE = H(m) for every trial -> spread exactly 0
+    res1 = gce.search(d(times), d(mags), d(offs), d(periods), d(pdots), 1, 10, top_k=0, want_cube=False, want_stats=True)
+    torch.cuda.synchronize()
+    s1 = res1.stats.cpu().numpy()
+    assert s1[2, 1] == 0.0 and s1[2, 0] == s1[2, 2] > 0 and np.isnan(s1[2, 3])
+    # a different CTA split (one light curve alone gets more jobs per light curve) gives the same bits
+    a, b = offs[2], offs[3]
+    res2 = gce.search(d(times[a:b]), d(mags[a:b]), d(np.array([0, b - a])), d(periods), d(pdots), 20, 10, top_k=0,
+                      want_cube=False, want_stats=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(res2.stats.cpu().numpy()[0], st[2])
+
+
+def test_c4_full_stats_sampled_light_curves(gce, oracle):
+    """configs[3] at full size in the no-cube mode with Eq. 5 fused: statistics of three light curves against the
+    oracle's full rows, the rest against bounds (min = best CE, 0 <= min <= mean <= ln n_m, std > 0)."""
+    w = W.make("C4")
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), 15, 8, top_k=5, want_cube=False,
+                     want_stats=True)
+    torch.cuda.synchronize()
+    st = res.stats.cpu().numpy()
+    assert np.all(st[:, 2] >= 0) and np.all(st[:, 2] <= st[:, 0]) and np.all(st[:, 0] <= np.log(8) + 1e-12)
+    assert np.all(st[:, 1] > 0) and np.all(st[:, 3] > 0)
+    assert np.allclose(st[:, 2], res.best_ce[:, 0].cpu().numpy().astype(np.float64), rtol=1e-6)
+    for lc in (0, 500, 999):
+        a, b = w.lc_offsets[lc], w.lc_offsets[lc + 1]
+        row = oracle.ce_search(w.times[a:b], w.mags[a:b], np.array([0, b - a]), w.periods, w.pdots, 15, 8)[0]
+        np.testing.assert_allclose(st[lc], _stats_ref(oracle, row.reshape(1, -1))[0], rtol=RTOL_STATS)
