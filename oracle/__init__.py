@@ -63,6 +63,9 @@ def lib():
                                            C.c_int32, C.c_int32, _f64p, C.c_int32]
         L.gce_oracle_ce_at.argtypes = [_f64p, _f64p, _i64p, C.c_int32, _f64p, C.c_int64, _f64p, C.c_int64,
                                        C.c_int32, C.c_int32, _i64p, C.c_int64, _f64p, C.c_int32]
+        L.gce_oracle_ce_search_overlap.argtypes = L.gce_oracle_ce_search.argtypes
+        L.gce_oracle_ce_at_overlap.argtypes = L.gce_oracle_ce_at.argtypes
+        L.gce_oracle_overlap_counts.argtypes = [_i64p, C.c_int32, C.c_int32, _i64p]
         L.gce_oracle_topk.argtypes = [_f64p, C.c_int64, C.c_int32, _i64p, _f64p]
         L.gce_oracle_significance.argtypes = [_f64p, C.c_int64, _f64p]
         L.gce_oracle_num_threads.restype = C.c_int
@@ -118,24 +121,34 @@ def histogram(times, mags, periods, pdots, n_phase_bins, n_mag_bins, trial_q):
     return out
 
 
-def ce_search(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, n_threads=0):
-    """Full CE cube [n_lc][n_p][n_pdot] (fp64)."""
+def overlap_counts(counts):
+    """N2: the 50 %-overlapping table c[k][i] = n[k][i] + n[k-1 mod n_phase][i] from plain counts n[j][i]."""
+    cnt = _i64(counts)
+    out = np.empty_like(cnt)
+    _check(lib().gce_oracle_overlap_counts(_p(cnt, _i64p), cnt.shape[0], cnt.shape[1], _p(out, _i64p)))
+    return out
+
+
+def ce_search(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, n_threads=0, overlap=False):
+    """Full CE cube [n_lc][n_p][n_pdot] (fp64).  overlap=True: 50 %-overlapping phase bins (N2)."""
     t, m, offs, periods, pdots = _f64(times), _f64(mags), _i64(lc_offsets), _f64(periods), _f64(pdots)
     n_lc = offs.shape[0] - 1
     out = np.empty((n_lc, periods.shape[0], pdots.shape[0]), dtype=np.float64)
-    _check(lib().gce_oracle_ce_search(_p(t, _f64p), _p(m, _f64p), _p(offs, _i64p), n_lc,
+    fn = lib().gce_oracle_ce_search_overlap if overlap else lib().gce_oracle_ce_search
+    _check(fn(_p(t, _f64p), _p(m, _f64p), _p(offs, _i64p), n_lc,
                                       _p(periods, _f64p), periods.shape[0], _p(pdots, _f64p), pdots.shape[0],
                                       int(n_phase_bins), int(n_mag_bins), _p(out, _f64p), int(n_threads)))
     return out
 
 
-def ce_at(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, trial_q, n_threads=0):
+def ce_at(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, trial_q, n_threads=0, overlap=False):
     """CE at sampled flat trials (same list for every light curve) -> [n_lc][n_trials] (fp64)."""
     t, m, offs, periods, pdots = _f64(times), _f64(mags), _i64(lc_offsets), _f64(periods), _f64(pdots)
     trial_q = _i64(trial_q)
     n_lc = offs.shape[0] - 1
     out = np.empty((n_lc, trial_q.shape[0]), dtype=np.float64)
-    _check(lib().gce_oracle_ce_at(_p(t, _f64p), _p(m, _f64p), _p(offs, _i64p), n_lc,
+    fn = lib().gce_oracle_ce_at_overlap if overlap else lib().gce_oracle_ce_at
+    _check(fn(_p(t, _f64p), _p(m, _f64p), _p(offs, _i64p), n_lc,
                                   _p(periods, _f64p), periods.shape[0], _p(pdots, _f64p), pdots.shape[0],
                                   int(n_phase_bins), int(n_mag_bins), _p(trial_q, _i64p), trial_q.shape[0],
                                   _p(out, _f64p), int(n_threads)))

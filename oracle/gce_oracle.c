@@ -30,7 +30,8 @@
  * Pins (tests/test_oracle_pins.py, all -m "not gpu"): dyadic hand folds, hand count tables
  * with closed-form CE (0, ln 2, 1/2 ln 2, 0.6059391565991873), scipy.stats.entropy identity
  * H(m,phi) - H(phi), exact rational refold, Eq. 6 closed form, numpy.histogram marginals,
- * invariants 0 <= CE <= H(m), noiseless recovery.  Parity with a CE value printed in the
+ * invariants 0 <= CE <= H(m), noiseless recovery; N2 overlap: hand tables, exact-rational interval
+ * membership, CE_plain <= CE_overlap <= CE_plain + ln 2.  Parity with a CE value printed in the
  * paper: UNPINNED (the paper prints none).
  */
 #include <math.h>
@@ -169,9 +170,36 @@ int gce_oracle_histogram(const double *dt, const double *dt2, const int32_t *mbi
  * The search: every light curve x every (P, Pdot).  out_ce layout [n_lc][n_p][n_pdot],
  * Pdot fastest (Q10).  OpenMP over periods; each thread has its own count table.
  * ------------------------------------------------------------------------------------- */
-int gce_oracle_ce_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
-                         const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                         int32_t n_phase, int32_t n_mag, double *out_ce, int32_t n_threads)
+/* ---------------------------------------------------------------------------------------
+ * NEXT item N2 -- 50 % overlapping phase bins ("each histogram bin has a 50% overlap
+ * with each adjacent bin", Fig. 3 caption :162 "50 phase bins that overlap by 50% with surrounding
+ * bins").  Reading Q3: phase axis only, cyclic.  The n_phase bins have
+ * width 2/n_phase and start 1/n_phase apart: bin k covers the phases [(k-1)/n_phase, (k+1)/n_phase)
+ * (mod 1), i.e. the two cells k-1 and k of the plain n_phase-cell grid of S2/S3.  Every point
+ * therefore lies in exactly two bins, the table holds 2N entries, and probabilities are
+ * normalised by 2N:  c[k][i] = n[k][i] + n[k-1 mod n_phase][i].  Eq. 4 is then applied to c.
+ * ------------------------------------------------------------------------------------- */
+int gce_oracle_overlap_counts(const int64_t *cnt, int32_t n_phase, int32_t n_mag, int64_t *out)
+{
+    if (n_phase < 1 || n_mag < 1) return GCE_ORACLE_EINVAL;
+    for (int32_t k = 0; k < n_phase; ++k) {
+        const int32_t km = (k + n_phase - 1) % n_phase;
+        for (int32_t i = 0; i < n_mag; ++i)
+            out[(int64_t)k * n_mag + i] = cnt[(int64_t)k * n_mag + i] + cnt[(int64_t)km * n_mag + i];
+    }
+    return GCE_ORACLE_OK;
+}
+
+static double ce_one_trial(const int64_t *cnt, int64_t *tmp, int32_t n_phase, int32_t n_mag, int64_t n, int overlap)
+{
+    if (!overlap) return gce_oracle_ce_from_counts(cnt, n_phase, n_mag, n);
+    gce_oracle_overlap_counts(cnt, n_phase, n_mag, tmp);
+    return gce_oracle_ce_from_counts(tmp, n_phase, n_mag, 2 * n);
+}
+
+static int ce_search_impl(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                          const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                          int32_t n_phase, int32_t n_mag, double *out_ce, int32_t n_threads, int overlap)
 {
     if (n_lc < 0 || n_p < 0 || n_pdot < 1 || n_phase < 1 || n_mag < 1) return GCE_ORACLE_EINVAL;
 #ifdef _OPENMP
@@ -187,12 +215,13 @@ int gce_oracle_ce_search(const double *times, const double *mags, const int64_t 
         double *ce_l = out_ce + (int64_t)l * n_p * n_pdot;
 #pragma omp parallel
         {
-            int64_t *cnt = (int64_t *)malloc(sizeof(int64_t) * (size_t)n_phase * (size_t)n_mag);
+            int64_t *cnt = (int64_t *)malloc(sizeof(int64_t) * 2 * (size_t)n_phase * (size_t)n_mag);
+            int64_t *tmp = cnt + (size_t)n_phase * (size_t)n_mag;
 #pragma omp for schedule(static)
             for (int64_t ip = 0; ip < n_p; ++ip) {
                 for (int64_t ipd = 0; ipd < n_pdot; ++ipd) {
                     histogram_one_trial(dt, dt2, mbin, n, periods[ip], pdots[ipd], n_phase, n_mag, cnt);
-                    ce_l[ip * n_pdot + ipd] = gce_oracle_ce_from_counts(cnt, n_phase, n_mag, n);
+                    ce_l[ip * n_pdot + ipd] = ce_one_trial(cnt, tmp, n_phase, n_mag, n, overlap);
                 }
             }
             free(cnt);
@@ -202,12 +231,28 @@ int gce_oracle_ce_search(const double *times, const double *mags, const int64_t 
     return GCE_ORACLE_OK;
 }
 
+int gce_oracle_ce_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                         const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                         int32_t n_phase, int32_t n_mag, double *out_ce, int32_t n_threads)
+{
+    return ce_search_impl(times, mags, lc_offsets, n_lc, periods, n_p, pdots, n_pdot, n_phase, n_mag, out_ce,
+                          n_threads, 0);
+}
+
+int gce_oracle_ce_search_overlap(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                                 const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                                 int32_t n_phase, int32_t n_mag, double *out_ce, int32_t n_threads)
+{
+    return ce_search_impl(times, mags, lc_offsets, n_lc, periods, n_p, pdots, n_pdot, n_phase, n_mag, out_ce,
+                          n_threads, 1);
+}
+
 /* CE at a list of flat trial indices (the same list for every light curve): sampled parity at
  * full-size grids.  out_ce layout [n_lc][n_trials]. */
-int gce_oracle_ce_at(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
-                     const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                     int32_t n_phase, int32_t n_mag, const int64_t *trial_q, int64_t n_trials,
-                     double *out_ce, int32_t n_threads)
+static int ce_at_impl(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                      const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                      int32_t n_phase, int32_t n_mag, const int64_t *trial_q, int64_t n_trials,
+                      double *out_ce, int32_t n_threads, int overlap)
 {
     if (n_lc < 0 || n_p < 0 || n_pdot < 1 || n_phase < 1 || n_mag < 1) return GCE_ORACLE_EINVAL;
     for (int64_t s = 0; s < n_trials; ++s)
@@ -224,18 +269,37 @@ int gce_oracle_ce_at(const double *times, const double *mags, const int64_t *lc_
         gce_oracle_preprocess(times + off, mags + off, n, n_mag, dt, dt2, mbin);
 #pragma omp parallel
         {
-            int64_t *cnt = (int64_t *)malloc(sizeof(int64_t) * (size_t)n_phase * (size_t)n_mag);
+            int64_t *cnt = (int64_t *)malloc(sizeof(int64_t) * 2 * (size_t)n_phase * (size_t)n_mag);
+            int64_t *tmp = cnt + (size_t)n_phase * (size_t)n_mag;
 #pragma omp for schedule(static)
             for (int64_t s = 0; s < n_trials; ++s) {
                 const int64_t q = trial_q[s];
                 histogram_one_trial(dt, dt2, mbin, n, periods[q / n_pdot], pdots[q % n_pdot], n_phase, n_mag, cnt);
-                out_ce[(int64_t)l * n_trials + s] = gce_oracle_ce_from_counts(cnt, n_phase, n_mag, n);
+                out_ce[(int64_t)l * n_trials + s] = ce_one_trial(cnt, tmp, n_phase, n_mag, n, overlap);
             }
             free(cnt);
         }
         free(dt); free(dt2); free(mbin);
     }
     return GCE_ORACLE_OK;
+}
+
+int gce_oracle_ce_at(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                     const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                     int32_t n_phase, int32_t n_mag, const int64_t *trial_q, int64_t n_trials,
+                     double *out_ce, int32_t n_threads)
+{
+    return ce_at_impl(times, mags, lc_offsets, n_lc, periods, n_p, pdots, n_pdot, n_phase, n_mag, trial_q, n_trials,
+                      out_ce, n_threads, 0);
+}
+
+int gce_oracle_ce_at_overlap(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                             const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                             int32_t n_phase, int32_t n_mag, const int64_t *trial_q, int64_t n_trials,
+                             double *out_ce, int32_t n_threads)
+{
+    return ce_at_impl(times, mags, lc_offsets, n_lc, periods, n_p, pdots, n_pdot, n_phase, n_mag, trial_q, n_trials,
+                      out_ce, n_threads, 1);
 }
 
 /* ---------------------------------------------------------------------------------------

@@ -370,3 +370,97 @@ def test_significance_matches_numpy(oracle):
     assert mu == pytest.approx(ce.mean(), rel=1e-13)
     assert sigma == pytest.approx(ce.std(ddof=0), rel=1e-12)
     assert rho == pytest.approx((ce.mean() - 0.2) / ce.std(ddof=0), rel=1e-12)
+
+
+# ------------------------------------------------------------------ N2: 50 %-overlapping phase bins
+def _read_tables(fname):
+    tables, cur = [], None
+    for line in open(os.path.join(GOLDEN, fname)):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        tok = line.split()
+        if tok[0] == "table":
+            cur = {"name": tok[1], "rows": int(tok[3]), "cols": int(tok[5]), "expr": " ".join(tok[7:]), "cnt": []}
+            tables.append(cur)
+        else:
+            cur["cnt"].append([int(v) for v in tok])
+    return tables
+
+
+@pytest.mark.parametrize("tab", _read_tables("ce_overlap_hand_tables.txt"), ids=lambda t: t["name"])
+def test_overlap_hand_tables(oracle, tab):
+    n = np.array(tab["cnt"], dtype=np.int64)
+    assert n.shape == (tab["rows"], tab["cols"])
+    expect = eval(tab["expr"], {"log": math.log})
+    c = oracle.overlap_counts(n)
+    assert c.sum() == 2 * n.sum()
+    got = oracle.ce_from_counts(c)
+    assert got == pytest.approx(expect, rel=1e-14, abs=1e-16)
+    if expect == 0.0:
+        assert got == 0.0
+
+
+def _brute_overlap_counts(t, m, P, Pd, n_phase, n_mag):
+    """Independent definition by interval membership, exact rationals: bin k holds the points whose phase lies in the
+    cyclic interval [(k-1)/n_phase, (k+1)/n_phase) -- width 2/n_phase, 50 % shared with each neighbour."""
+    Ft = [Fraction(float(v)) for v in t]
+    Fm = [Fraction(float(v)) for v in m]
+    t0, lo, hi = min(Ft), min(Fm), max(Fm)
+    cnt = np.zeros((n_phase, n_mag), dtype=np.int64)
+    FP, FPd = Fraction(P), Fraction(Pd)
+    w = Fraction(1, n_phase)
+    for tk, mk in zip(Ft, Fm):
+        d = tk - t0
+        x = d / FP - FPd * d * d / (2 * FP * FP)
+        phi = x - math.floor(x)
+        i = 0 if hi == lo else min(math.floor((mk - lo) / (hi - lo) * n_mag), n_mag - 1)
+        for k in range(n_phase):
+            rel = (phi - (k - 1) * w) % 1          # distance past the bin's left edge, cyclic
+            if rel < 2 * w:
+                cnt[k, i] += 1
+    return cnt
+
+
+def test_overlap_counts_equal_interval_membership_brute_force(oracle):
+    """Dyadic inputs (fp64 exact): the oracle's overlapped table equals exact-rational interval membership, every
+    point is counted exactly twice, and the search's CE equals scipy's H(m,phi) - H(phi) of that table."""
+    rng = np.random.default_rng(31)
+    t = rng.integers(0, 4096, size=70).astype(np.float64) + 3.0
+    m = rng.integers(0, 64, size=70) / 64.0
+    periods = np.array([8.0, 4.0, 16.0, 32.0])
+    pdots = np.array([-0.5, 0.0, 0.25])
+    for n_phase, n_mag in ((8, 4), (16, 3), (4, 2)):
+        q = np.arange(periods.size * pdots.size)
+        plain = oracle.histogram(t, m, periods, pdots, n_phase, n_mag, q)
+        cube = oracle.ce_search(t, m, [0, 70], periods, pdots, n_phase, n_mag, overlap=True)
+        at = oracle.ce_at(t, m, [0, 70], periods, pdots, n_phase, n_mag, q, overlap=True)
+        for ip, P in enumerate(periods):
+            for ipd, Pd in enumerate(pdots):
+                ref = _brute_overlap_counts(t, m, P, Pd, n_phase, n_mag)
+                got = oracle.overlap_counts(plain[ip * pdots.size + ipd])
+                assert np.array_equal(got, ref), (n_phase, P, Pd)
+                assert ref.sum() == 140 and np.array_equal(ref.sum(axis=0), 2 * plain[0].sum(axis=0))
+                ce_ref = scipy.stats.entropy(ref.ravel()) - scipy.stats.entropy(ref.sum(axis=1))
+                assert cube[0, ip, ipd] == pytest.approx(ce_ref, rel=1e-12, abs=1e-14)
+                assert at[0, ip * pdots.size + ipd] == cube[0, ip, ipd]
+
+
+def test_overlap_special_cases_and_bounds(oracle):
+    """n_phase = 1 and 2: every bin holds every point -> CE = H(m); n_mag = 1 -> 0; 0 <= CE <= H(m); on a smooth
+    light curve at its true period the overlapped CE stays low and within ln 2 of the plain one
+    (each overlapped bin is the union of two plain cells)."""
+    w = W.make("C1", n_p=200)
+    _, _, mbin = oracle.preprocess(w.times, w.mags, 10)
+    hm = scipy.stats.entropy(np.bincount(mbin, minlength=10))
+    for n_phase in (1, 2):
+        ce = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, n_phase, 10, overlap=True)
+        assert np.allclose(ce, hm, rtol=1e-13)
+    assert np.all(oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 1, overlap=True) == 0.0)
+    ov = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 10, overlap=True)
+    pl = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 10)
+    assert np.all(ov >= 0) and np.all(ov <= hm + 1e-12)
+    # an overlapped bin's magnitude distribution is a two-component mixture of its cells' distributions, and every cell
+    # enters two bins with weight 1/2: H(mixture) >= the weighted mean of the parts (concavity) and <= that mean + ln 2
+    assert np.all(ov >= pl - 1e-12)
+    assert np.all(ov <= pl + math.log(2) + 1e-12)
