@@ -46,6 +46,7 @@ extern "C" {
 #define GCE_CE_MAX_BINS 64         /* n_phase_bins and n_mag_bins are each in 1..64                 */
 #define GCE_CE_MAX_TOPK 32         /* top_k is in 0..32                                             */
 #define GCE_CE_MAX_POINTS 65535    /* points per light curve (16-bit counters)                      */
+#define GCE_CE_MAX_POINTS_OVERLAP 32767 /* ... with overlap = 1 (the table holds 2N entries)            */
 
 typedef struct gce_ce_params {
     int32_t n_phase_bins; /* n_phi, 1..64                                                         */
@@ -53,7 +54,9 @@ typedef struct gce_ce_params {
     int32_t top_k;        /* 0 = no selection output; 1..32 = keep the k smallest CE per LC        */
     int32_t ce_fp64;      /* 0: out_ce is float[...]; 1: out_ce is double[...]                     */
     int32_t want_stats;   /* 1: out_stats receives the Eq. 5 statistics (requires out_stats)      */
-    int32_t overlap;      /* 0: plain bins (hot path).  1: 50 % overlapping phase bins (:106, N2)  */
+    int32_t overlap;      /* 0: plain bins (hot path).  1: 50 % overlapping phase bins (:106, :162):
+                           * n_phase_bins bins of width 2/n_phase_bins, bin k = plain cells k-1 and k (cyclic),
+                           * every point counted twice, p = c / 2N.  The debug calls ignore it.            */
     int32_t reserved[2];  /* must be 0                                                            */
     /* Optional cudaEvent_t handles (NULL = none), recorded on `stream` immediately before / after the
      * fold+bin+entropy kernel, so a harness can time the dominant kernel alone without a profiler.    */

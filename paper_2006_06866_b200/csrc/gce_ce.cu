@@ -74,6 +74,7 @@ struct SearchParams {
     int32_t ltab_n;
     int32_t top_k;
     int32_t ce_fp64;
+    int32_t overlap;           // N2: 50 %-overlapping phase bins
     void *out_ce;              // cube or NULL
     int64_t *part_S, *part_q;  // [n_lc][jobs_per_lc][top_k]
     uint64_t *part_stats;      // [n_lc][jobs_per_lc][kStatWords] partial Eq. 5 sums, or NULL
@@ -236,7 +237,7 @@ __device__ __forceinline__ MinMax3 block_minmax(MinMax3 v, MinMax3 *sh) {
 __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ times, const double *__restrict__ mags,
                                                     const int64_t *__restrict__ lc_offsets, int n_m,
                                                     double2 *__restrict__ pts, int32_t *__restrict__ seg,
-                                                    LcInfo *__restrict__ info, const int64_t *__restrict__ ltab) {
+                                                    LcInfo *__restrict__ info, const int64_t *__restrict__ ltab, const int mult) {
     __shared__ MinMax3 sh_red[8];
     __shared__ int sh_cnt[GCE_CE_MAX_BINS + 1];
     __shared__ int sh_cur[GCE_CE_MAX_BINS];
@@ -262,13 +263,13 @@ __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ t
     __syncthreads();
     if (threadIdx.x == 0) {
         int acc = 0;
-        int64_t K = ltab[n];
+        int64_t K = ltab[mult * n];  // mult = 2 with overlapping phase bins: the table holds 2N entries
         for (int i = 0; i < n_m; ++i) {
             const int c = sh_cnt[i];
             seg[(int64_t)lc * (n_m + 1) + i] = acc;
             sh_cur[i] = acc;
             acc += c;
-            K -= ltab[c];
+            K -= ltab[mult * c];
         }
         info[lc].K = K;
         seg[(int64_t)lc * (n_m + 1) + n_m] = acc;
@@ -404,13 +405,17 @@ __device__ __forceinline__ void close_word(const uint32_t w, const int j, const 
 // set of counter rows in shared memory updated with one RED per word (no registers, so more threads fit per SM).
 // With a compile-time n_phi the read-and-clear atomics of kCloseGroup phase bins are issued back to back before
 // their results are used, so their latency overlaps.
-template <int NPHI, bool REGM, int R, bool DUMP, bool BIG>
+// OVL (NEXT item N2): 50 %-overlapping phase bins -- bin k holds the plain cells k-1 and k (cyclic), so
+// the looked-up count is w[k] + w[k-1] (packed 16-bit pairs; needs 2N <= 65535); the folds and the plain marginal are
+// unchanged, the overlap costs one add per word.
+template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL>
 __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off,
                                               const uint32_t (&hb)[(R + 1) / 2],
                                               uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
                                               const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
                                               const int64_t s0, const bool (&valid)[R], const int seg_i) {
     constexpr int RW = (R + 1) / 2;
+    uint32_t prev[RW], first[RW];
     if (NPHI > 0) {
         constexpr int NP = NPHI > 0 ? NPHI : 1;
         constexpr int G = NP % kCloseGroup == 0 ? kCloseGroup : 1;
@@ -425,20 +430,36 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
             for (int jj = 0; jj < G; ++jj)
 #pragma unroll
                 for (int w2 = 0; w2 < RW; ++w2) {
-                    if (REGM) mg[REGM ? j0 + jj : 0][w2] += w[jj][w2];
-                    else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, w[jj][w2]);
-                    close_word<R, DUMP, BIG>(w[jj][w2], j0 + jj, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                    const uint32_t ww = w[jj][w2];
+                    if (REGM) mg[REGM ? j0 + jj : 0][w2] += ww;
+                    else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, ww);
+                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                    else {
+                        if (j0 + jj == 0) first[w2] = ww;
+                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                        prev[w2] = ww;
+                    }
                 }
         }
     } else {
         for (int j = 0; j < n_phi; ++j) {
 #pragma unroll
             for (int w2 = 0; w2 < RW; ++w2) {
-                const uint32_t w = fetch_word(j, n_phi, rs, hb[w2]);
-                red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, w);
-                close_word<R, DUMP, BIG>(w, j, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                const uint32_t ww = fetch_word(j, n_phi, rs, hb[w2]);
+                red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, ww);
+                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                else {
+                    if (j == 0) first[w2] = ww;
+                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                    prev[w2] = ww;
+                }
             }
         }
+    }
+    if (OVL) {  // bin 0 = cells n_phi-1 and 0
+#pragma unroll
+        for (int w2 = 0; w2 < RW; ++w2)
+            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
     }
 }
 
@@ -517,7 +538,8 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     uint32_t hb[RW];
 #pragma unroll
     for (int w2 = 0; w2 < RW; ++w2) hb[w2] = smem_u32(hist) + (uint32_t)tid * 4u + (uint32_t)w2 * plane;
-    const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)N : 0.0;
+    const bool ovl = !DUMP && prm.overlap != 0;  // N2: 2N table entries per trial
+    const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)(ovl ? 2 * N : N) : 0.0;
     uint32_t mg[NPHI_REG][RW];  // phase marginal n_j of the R trials (NPHI > 0), packed like the histogram
 #pragma unroll
     for (int j = 0; j < NPHI_REG; ++j)
@@ -589,10 +611,18 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 if (b1 > k_end) break;  // the bin continues in the next buffer
                 // ---------------- S4: the bin is complete; a cell holds at most b1 - b0 points
                 if (b1 > b0) {
-                    if (b1 - b0 < kLtabSmem)
-                        close_mag_bin<NPHI, REGM, R, DUMP, false>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
-                    else
-                        close_mag_bin<NPHI, REGM, R, DUMP, true>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                    // a cell of this bin holds at most b1 - b0 points (twice that with overlapping bins)
+                    if (!ovl) {
+                        if (b1 - b0 < kLtabSmem)
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, false>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        else
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, false>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                    } else if (!DUMP) {
+                        if (2 * (b1 - b0) < kLtabSmem)
+                            close_mag_bin<NPHI, REGM, R, false, false, true>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        else
+                            close_mag_bin<NPHI, REGM, R, false, true, true>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                    }
                 }
                 ++seg_s;
             }
@@ -614,19 +644,35 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 S1[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
                 if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
             };
-            auto marg_pass = [&](auto big) {
+            auto marg_pass = [&](auto big, auto ovlt) {
+                constexpr bool OVL = decltype(ovlt)::value;
+                uint32_t prev[RW], first[RW];
                 if (REGM) {
 #pragma unroll
                     for (int j = 0; j < NPHI_REG; ++j)
 #pragma unroll
-                        for (int w2 = 0; w2 < RW; ++w2) { add_marg(mg[j][w2], w2, big); mg[j][w2] = 0u; }
+                        for (int w2 = 0; w2 < RW; ++w2) {
+                            const uint32_t ww = mg[j][w2];
+                            mg[j][w2] = 0u;
+                            if (!OVL) add_marg(ww, w2, big);
+                            else { if (j == 0) first[w2] = ww; else add_marg(ww + prev[w2], w2, big); prev[w2] = ww; }
+                        }
                 } else {
                     for (int j = 0; j < n_phi; ++j)
 #pragma unroll
-                        for (int w2 = 0; w2 < RW; ++w2) add_marg(exch0_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs), w2, big);
+                        for (int w2 = 0; w2 < RW; ++w2) {
+                            const uint32_t ww = exch0_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs);
+                            if (!OVL) add_marg(ww, w2, big);
+                            else { if (j == 0) first[w2] = ww; else add_marg(ww + prev[w2], w2, big); prev[w2] = ww; }
+                        }
+                }
+                if (OVL) {
+#pragma unroll
+                    for (int w2 = 0; w2 < RW; ++w2) add_marg(first[w2] + prev[w2], w2, big);
                 }
             };
-            if (N < kLtabSmem) marg_pass(FalseT{}); else marg_pass(TrueT{});
+            if (!ovl) { if (N < kLtabSmem) marg_pass(FalseT{}, FalseT{}); else marg_pass(TrueT{}, FalseT{}); }
+            else { if (2 * N < kLtabSmem) marg_pass(FalseT{}, TrueT{}); else marg_pass(TrueT{}, TrueT{}); }
         }
         double ce[R];
         int64_t S[R];
@@ -728,7 +774,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
 
 // One warp per light curve: merge jobs_per_lc x k candidates, write the user-facing selection.
 __global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ part_S, const int64_t *__restrict__ part_q,
-                                                   const LcInfo *__restrict__ info, int jobs_per_lc, int K,
+                                                   const LcInfo *__restrict__ info, int jobs_per_lc, int K, int mult,
                                                    int64_t *__restrict__ out_idx, float *__restrict__ out_ce) {
     const int lc = blockIdx.x, lane = threadIdx.x;
     WarpTopK top;
@@ -744,7 +790,7 @@ __global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ p
         const bool have = top.S != kInfS;
         const int n = info[lc].n;
         out_idx[(int64_t)lc * K + lane] = have ? top.q : -1;
-        if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)n)) : CUDART_NAN_F;
+        if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)(mult * n))) : CUDART_NAN_F;
     }
 }
 
@@ -755,7 +801,7 @@ __device__ __forceinline__ double u128_to_double(u128_t v) {
     return (double)(uint64_t)(v >> 64) * 18446744073709551616.0 + (double)(uint64_t)v;
 }
 __global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__ part, const LcInfo *__restrict__ info,
-                                                    int jobs_per_lc, double *__restrict__ out_stats) {
+                                                    int jobs_per_lc, int mult, double *__restrict__ out_stats) {
     __shared__ uint64_t sh[32][kStatWords];
     const int lc = blockIdx.x, lane = threadIdx.x;
     uint64_t acc[kStatWords];
@@ -773,7 +819,7 @@ __global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__
     const bool neg = (acc[2] >> 63) != 0;
     const double sum_d = neg ? -u128_to_double((u128_t)0 - A) : u128_to_double(A);
     const double sum_d2 = (double)acc[5] * 3.4028236692093846e38 + u128_to_double(((u128_t)acc[4] << 64) | acc[3]);
-    const double scale = ldexp(1.0, -kLfixShift) / (double)n_pts;
+    const double scale = ldexp(1.0, -kLfixShift) / (double)(mult * n_pts);
     const double mean_d = sum_d / n;
     double var = sum_d2 / n - mean_d * mean_d;
     if (var < 0.0 || acc[6] == acc[7]) var = 0.0;  // min == max: every trial has the same CE, the spread is exactly 0
@@ -916,7 +962,8 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     L.pts = o; o = align_up(o + sizeof(double2) * (size_t)(total_points > 0 ? total_points : 1), 256);
     L.seg = o; o = align_up(o + sizeof(int32_t) * (size_t)(n_lc > 0 ? n_lc : 1) * (prm->n_mag_bins + 1), 256);
     L.info = o; o = align_up(o + sizeof(LcInfo) * (size_t)(n_lc > 0 ? n_lc : 1), 256);
-    int64_t tn = total_points < GCE_CE_MAX_POINTS ? total_points : GCE_CE_MAX_POINTS;
+    int64_t tn = (prm->overlap ? 2 : 1) * total_points;  // largest count looked up: N, or 2N with overlapping bins
+    if (tn > GCE_CE_MAX_POINTS) tn = GCE_CE_MAX_POINTS;
     L.ltab_n = (int)tn + 1;
     L.ltab = o; o = align_up(o + sizeof(int64_t) * (size_t)L.ltab_n, 256);
     const Plan p = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins, dump);
@@ -936,7 +983,7 @@ int check_params(const gce_ce_params *prm) {
     if (prm->top_k < 0 || prm->top_k > GCE_CE_MAX_TOPK) return GCE_CE_ERR_RANGE;
     if (prm->ce_fp64 != 0 && prm->ce_fp64 != 1) return GCE_CE_ERR_RANGE;
     if (prm->want_stats != 0 && prm->want_stats != 1) return GCE_CE_ERR_RANGE;
-    if (prm->overlap != 0) return GCE_CE_ERR_RANGE;  // NEXT item N2: not yet built
+    if (prm->overlap != 0 && prm->overlap != 1) return GCE_CE_ERR_RANGE;
     if (prm->reserved[0] != 0 || prm->reserved[1] != 0) return GCE_CE_ERR_RANGE;
     return GCE_CE_OK;
 }
@@ -1055,7 +1102,8 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     }
     const int64_t n_trials = dump ? n_dump : n_p * n_pdot;
     gce_ce_params lay_prm = *prm;
-    if (dump) { lay_prm.top_k = 0; lay_prm.want_stats = 0; }
+    if (dump) { lay_prm.top_k = 0; lay_prm.want_stats = 0; lay_prm.overlap = 0; }  // the debug dump is always the plain table
+    const int mult = lay_prm.overlap ? 2 : 1;
     const Layout L = make_layout(total_points, n_lc, n_trials, dump ? 1 : n_pdot, &lay_prm, dump);
     if (workspace_bytes < L.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return GCE_CE_ERR_WORKSPACE;
     if (n_lc == 0) return GCE_CE_OK;
@@ -1070,7 +1118,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     k_ltab<<<(L.ltab_n + 255) / 256, 256, 0, st>>>(ltab, L.ltab_n);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
-    k_preprocess<<<n_lc, 256, 0, st>>>(times, mags, lc_offsets, prm->n_mag_bins, pts, seg, info, ltab);
+    k_preprocess<<<n_lc, 256, 0, st>>>(times, mags, lc_offsets, prm->n_mag_bins, pts, seg, info, ltab, mult);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
 
@@ -1087,6 +1135,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.ltab_n = L.ltab_n;
     sp.top_k = dump ? 0 : prm->top_k;
     sp.ce_fp64 = prm->ce_fp64;
+    sp.overlap = lay_prm.overlap;
     sp.out_ce = out_ce;
     sp.part_S = reinterpret_cast<int64_t *>(ws + L.part_S);
     sp.part_q = reinterpret_cast<int64_t *>(ws + L.part_q);
@@ -1106,13 +1155,13 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
         if (e != cudaSuccess) return cuda_fail(e);
     }
     if (!dump && prm->top_k > 0) {
-        k_merge_topk<<<n_lc, 32, 0, st>>>(sp.part_S, sp.part_q, info, n_trials > 0 ? plan.jobs_per_lc : 0, prm->top_k,
+        k_merge_topk<<<n_lc, 32, 0, st>>>(sp.part_S, sp.part_q, info, n_trials > 0 ? plan.jobs_per_lc : 0, prm->top_k, mult,
                                           out_best_idx, out_best_ce);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e);
     }
     if (!dump && prm->want_stats) {
-        k_merge_stats<<<n_lc, 32, 0, st>>>(sp.part_stats, info, n_trials > 0 ? plan.jobs_per_lc : 0, out_stats);
+        k_merge_stats<<<n_lc, 32, 0, st>>>(sp.part_stats, info, n_trials > 0 ? plan.jobs_per_lc : 0, mult, out_stats);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e);
     }

@@ -257,3 +257,62 @@ def test_c4_full_stats_sampled_light_curves(gce, oracle):
         a, b = w.lc_offsets[lc], w.lc_offsets[lc + 1]
         row = oracle.ce_search(w.times[a:b], w.mags[a:b], np.array([0, b - a]), w.periods, w.pdots, 15, 8)[0]
         np.testing.assert_allclose(st[lc], _stats_ref(oracle, row.reshape(1, -1))[0], rtol=RTOL_STATS)
+
+
+# ------------------------------------------------------------------------------------------ N2: 50 %-overlapping phase bins
+@pytest.mark.parametrize("name,kw,n_phi,n_m,k", [
+    ("C3", dict(n_lc=3, n_p=900, n_pdot=64), 50, 10, 4),     # the paper's production binning: generic n_phi
+    ("C3", dict(n_lc=2, n_p=1111, n_pdot=7), 50, 10, 1),     # trials of a thread do not share a period
+    ("C3", dict(n_lc=3, n_p=1500, n_pdot=64), 20, 10, 3),    # compile-time n_phi, register marginals
+    ("C2", dict(n_lc=6, n_p=3000), 50, 10, 1),               # Pdot = {0}
+    ("C4", dict(n_lc=9, n_p=5000), 15, 8, 5),
+    ("C5", dict(n_lc=2, n_p=300, n_pdot=16), 30, 10, 16),    # 2 x points per magnitude bin above the shared table
+    ("C1", dict(), 1, 10, 1), ("C1", dict(), 2, 10, 1), ("C1", dict(), 64, 64, 2),
+])
+def test_overlapping_phase_bins_match_oracle(gce, oracle, name, kw, n_phi, n_m, k):
+    """overlap = 1 against the oracle's N2 variant (bin k = plain cells k-1 and k, 2N entries): whole fp64 / fp32 cube,
+    fused top-k and Eq. 5 statistics."""
+    w = W.make(name, **kw)
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, n_phi, n_m, overlap=True)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    args = (d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), n_phi, n_m)
+    for fp64, rtol in ((True, RTOL64), (False, RTOL32)):
+        res = gce.search(*args, top_k=k, want_cube=True, ce_fp64=fp64, want_stats=True, overlap=True)
+        torch.cuda.synchronize()
+        assert_ce_close(res.ce.cpu().numpy(), ref, rtol)
+        for lc in range(w.n_lc):
+            assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), k, rtol, oracle)
+    want = _stats_ref(oracle, ref.reshape(w.n_lc, -1))
+    got = res.stats.cpu().numpy()
+    # constant CE (n_phi = 1 or 2: every bin holds every point): the oracle's two-pass sigma is rounding noise of
+    # order 1e-14, the GPU's integer sums give exactly 0 and rho = NaN; compare mean and min there
+    ok = want[:, 1] > 1e-10 * np.abs(want[:, 0])
+    np.testing.assert_allclose(got[ok], want[ok], rtol=RTOL_STATS, atol=1e-13)
+    np.testing.assert_allclose(got[~ok][:, [0, 2]], want[~ok][:, [0, 2]], rtol=RTOL_STATS, atol=1e-13)
+    assert np.all(got[~ok][:, 1] == 0.0)
+    # the plain search on the same inputs is unchanged by the option and never above the overlapped CE
+    plain = gce.search(*args, top_k=0, want_cube=True, ce_fp64=True)
+    torch.cuda.synchronize()
+    assert bool(torch.all(res.ce.double() >= plain.ce - 1e-5))
+
+
+def test_overlap_paper_binning_sampled_at_c3_size(gce, oracle):
+    """The paper's production setting (50 overlapping phase bins x 10 magnitude bins) on the full C3
+    grid without a cube: sampled oracle values against the reported best, selection properties."""
+    w = W.make("C3")
+    w.n_phase_bins, w.n_mag_bins = 50, 10
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), 50, 10, top_k=3, want_cube=False,
+                     want_stats=True, overlap=True)
+    torch.cuda.synchronize()
+    idx = res.best_idx.cpu().numpy()
+    val = res.best_ce.cpu().numpy()
+    q = sample_trials(w.periods.size * w.pdots.size, 1500, seed=77)
+    ref = oracle.ce_at(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 50, 10, q, overlap=True)
+    for lc in range(w.n_lc):
+        exact = oracle.ce_at(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 50, 10, idx[lc], overlap=True)[lc]
+        assert np.all(np.abs(val[lc] - exact) <= RTOL32 * np.abs(exact) + 1e-12)
+        better = ref[lc] < exact[-1] * (1 - RTOL64) - 1e-13
+        assert set(q[better].tolist()) <= set(idx[lc].tolist())
+    st = res.stats.cpu().numpy()
+    assert np.allclose(st[:, 2], val[:, 0].astype(np.float64), rtol=1e-6) and np.all(st[:, 1] > 0)
