@@ -43,6 +43,7 @@ METRIC = "CE point-folds/sec"
 UNIT = "point-folds/s"
 FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (probe-measured)
 N_SM = 148
+OVERLAP = [False]   # set from --overlap; the oracle legs time the same binning
 # DRAM traffic of one k_search launch from the committed ncu --set full capture (profiles/r1_k_search_C3_full.md):
 # 17.1 MB read + 773.2 MB written; the algorithmic output is the 819.2 MB fp32 cube (part of it is still in L2 at
 # kernel end).  Only workloads that were captured have an entry.
@@ -118,6 +119,16 @@ def make_workload(name, rank, shrink):
     return W.make(name, **kw)
 
 
+def apply_binning(w, args):
+    """--n-phase-bins / --n-mag-bins / --overlap: the same light curves and grid with another binning, e.g. the paper's
+    production setting 50 overlapping phase bins x 10.  Named in config; never the default."""
+    if args.n_phase_bins:
+        w.n_phase_bins = args.n_phase_bins
+    if args.n_mag_bins:
+        w.n_mag_bins = args.n_mag_bins
+    return w
+
+
 def algorithmic_fp64_ops_per_pointfold(w):
     """DMUL a=dt*invP (shared by the Pdot values of one period), DMUL b=dt2*c, DADD x=a+b,
     DMUL y=x*n_phi, DADD.RD floor  ->  4 + 1/n_pdot per point-fold; 3 when the grid is Pdot = {0} only."""
@@ -135,7 +146,8 @@ def oracle_sample(w, seconds_target):
     n_cal = max(1, min(w.n_p, int(2e8 // max(1, w.total_points * w.n_pdot))))
     cal = w.subset(p_idx=np.linspace(0, w.n_p - 1, n_cal).astype(np.int64))
     t = time.perf_counter()
-    oracle.ce_search(cal.times, cal.mags, cal.lc_offsets, cal.periods, cal.pdots, w.n_phase_bins, w.n_mag_bins)
+    oracle.ce_search(cal.times, cal.mags, cal.lc_offsets, cal.periods, cal.pdots, w.n_phase_bins, w.n_mag_bins,
+                     overlap=OVERLAP[0])
     dt = max(time.perf_counter() - t, 1e-4)
     rate = cal.point_folds / dt
     n_s = int(min(w.n_p, max(n_cal, rate * seconds_target // max(1, w.total_points * w.n_pdot))))
@@ -147,7 +159,7 @@ def time_oracle(sample, w):
     import oracle
     t = time.perf_counter()
     oracle.ce_search(sample.times, sample.mags, sample.lc_offsets, sample.periods, sample.pdots,
-                     w.n_phase_bins, w.n_mag_bins)
+                     w.n_phase_bins, w.n_mag_bins, overlap=OVERLAP[0])
     return time.perf_counter() - t
 
 
@@ -156,7 +168,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     import oracle
-    w = make_workload(args.config, 0, args.quick)
+    w = apply_binning(make_workload(args.config, 0, args.quick), args)
     per_step = max(1.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
     sample, desc = oracle_sample(w, per_step)
     for _ in range(args.warmup):
@@ -178,7 +190,7 @@ def run_reference(args):
 def workload_config(w, args):
     return {"workload": f"{w.name} (BASELINE.json:configs[{int(w.name[1]) - 1}])" + (" QUICK-SHRUNK" if args.quick else ""),
             "n_lc": w.n_lc, "n_obs_total": w.total_points, "n_p": w.n_p, "n_pdot": w.n_pdot,
-            "n_phase_bins": w.n_phase_bins, "n_mag_bins": w.n_mag_bins, "top_k": w.top_k, "ce_cube": bool(w.want_cube),
+            "n_phase_bins": w.n_phase_bins, "n_mag_bins": w.n_mag_bins, "overlap": bool(args.overlap), "top_k": w.top_k, "ce_cube": bool(w.want_cube),
             "point_folds_per_step_per_gpu": w.point_folds, "parallelism": f"independent light-curve batches x{args.gpus}",
             "l2": "flushed between timed steps (256 MiB write), each step timed by its own CUDA-event pair"}
 
@@ -206,13 +218,13 @@ def run_ours(args):
         dist.barrier()
     import paper_2006_06866_b200 as gce
 
-    w = make_workload(args.config, rank, args.quick)
+    w = apply_binning(make_workload(args.config, rank, args.quick), args)
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     times, mags, offs, periods, pdots = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
     k = w.top_k
     ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev_a.record(); ev_b.record()  # forces creation of the cudaEvent_t handles
-    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k, ev_search_begin=ev_a, ev_search_end=ev_b)
+    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k, overlap=args.overlap, ev_search_begin=ev_a, ev_search_end=ev_b)
     ce = torch.empty((w.n_lc, w.n_p, w.n_pdot), dtype=torch.float32, device=dev) if w.want_cube else None
     bidx = torch.empty((w.n_lc, k), dtype=torch.int64, device=dev) if k else None
     bce = torch.empty((w.n_lc, k), dtype=torch.float32, device=dev) if k else None
@@ -264,7 +276,7 @@ def run_ours(args):
     h_ce = torch.empty((w.n_lc, w.n_p, w.n_pdot), dtype=torch.float32).pin_memory() if w.want_cube else None
     h_idx = torch.empty((w.n_lc, k), dtype=torch.int64).pin_memory() if k else None
     h_bce = torch.empty((w.n_lc, k), dtype=torch.float32).pin_memory() if k else None
-    prm_h = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k)
+    prm_h = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k, overlap=args.overlap)
     h2d = sum(x.numel() * x.element_size() for x in h_in)
     d2h = sum(x.numel() * x.element_size() for x in (h_ce, h_idx, h_bce) if x is not None)
     n_e2e = max(1, min(args.steps, 5))
@@ -336,8 +348,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true", help="shrunk grid, to test the bench itself; not a reportable number")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--n-phase-bins", type=int, default=0, help="override the config's phase bin count (named in config)")
+    ap.add_argument("--n-mag-bins", type=int, default=0, help="override the config's magnitude bin count")
+    ap.add_argument("--overlap", action="store_true", help="50 %% overlapping phase bins (N2, PAPER.md:106)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    OVERLAP[0] = bool(args.overlap)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -908,7 +908,10 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     else if (n_pdot % 2 == 0) { p.R = 2; p.share_p = true; }
     else { p.R = 4; p.share_p = false; }
     const int64_t avail = (int64_t)kSmemLimit - (int64_t)search_smem_fixed();
-    const bool templ = !dump && (n_phi == 15 || n_phi == 20 || n_phi == 30);
+    const bool templ = !dump && (n_phi == 15 || n_phi == 20 || n_phi == 30 || n_phi == 50);
+    // 50 phase bins (the paper's production binning): the register marginal of R = 4 trials would take
+    // 100 registers, so a thread owns R = 2 trials and 512 threads still fit (measured 2x the generic variant)
+    if (!dump && n_phi == 50) { p.R = 2; p.share_p = (n_pdot % 2 == 0); }
     // point buffer wanted: the average light curve plus a quarter (the per-LC lengths live on the device; a longer
     // light curve is streamed through the buffer in two halves instead of staying resident)
     const int64_t avg = n_lc > 0 ? (total_points + n_lc - 1) / n_lc : 0;
@@ -1038,6 +1041,11 @@ int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t
         case 15: return plan.regm ? launch_search_variant<15, true>(sp, plan, n_lc, st) : launch_search_variant<15, false>(sp, plan, n_lc, st);
         case 20: return plan.regm ? launch_search_variant<20, true>(sp, plan, n_lc, st) : launch_search_variant<20, false>(sp, plan, n_lc, st);
         case 30: return plan.regm ? launch_search_variant<30, true>(sp, plan, n_lc, st) : launch_search_variant<30, false>(sp, plan, n_lc, st);
+        case 50:
+            if (plan.regm && plan.R == 2)
+                return plan.share_p ? launch_search<50, true, 2, true, false>(sp, plan, n_lc, st)
+                                    : launch_search<50, true, 2, false, false>(sp, plan, n_lc, st);
+            return launch_search_variant<0, false>(sp, plan, n_lc, st);
         default: return launch_search_variant<0, false>(sp, plan, n_lc, st);
     }
 }
