@@ -42,7 +42,7 @@ constexpr int kLfixShift = 42;    // L table fixed point: 2^-42
 constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(y) in the low mantissa word
 constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
 constexpr int64_t kInfS = INT64_MAX;
-constexpr int kSmemLimit = 227 * 1024;
+constexpr int kSmemLimit = 227 * 1024 - 8 * kLtabSmem;  // dynamic shared memory per CTA: 227 KB minus the static L table
 constexpr int kStatWords = 8;     // partial Eq. 5 sums: n, sum d (i128), sum d^2 (u192), min S, pad; d = S - K
 constexpr int kMaxWarps = 20;     // warps per CTA of the largest variant (640 threads)
 constexpr int kCloseGroup = 5;    // phase bins whose read-and-clear atomics are in flight together in S4
@@ -304,15 +304,25 @@ __device__ __forceinline__ uint32_t exch0_u32(uint32_t addr) {
     return w;
 }
 
-// L(k) = k ln k in 2^-42 fixed point.  BIG = false: the caller guarantees c < kLtabSmem (a bound on the number of
-// points that can be in the cell), one LDS.64.  BIG = true: first kLtabSmem entries from shared memory, the rest
-// from global.
+// L(k) = k ln k in 2^-42 fixed point for the two 16-bit counter fields of a word.  The fields count in units of
+// 2^us: us = 3 whenever every count of the light curve fits 13 bits (N, or 2N with overlapping bins, <= 8191), so that a
+// field IS the byte offset of its table entry.  BIG = false: the caller guarantees us == 3 and counts < kLtabSmem (a
+// bound on the number of points that can be in the cell): mask / shift, one LDS.64 each.  BIG = true: any us, first
+// kLtabSmem entries from shared memory, the rest from global.
 template <bool BIG>
-__device__ __forceinline__ int64_t ltab_at(const int64_t *__restrict__ sL, const int64_t *__restrict__ gL, uint32_t c) {
-    if (!BIG) return sL[c];
-    int64_t v = sL[c & (kLtabSmem - 1)];
-    if (c >= (uint32_t)kLtabSmem) v = gL[c];
-    return v;
+__device__ __forceinline__ void ltab_pair(const int64_t *__restrict__ sL, const int64_t *__restrict__ gL, const uint32_t w,
+                                          const uint32_t us, int64_t &v0, int64_t &v1) {
+    if (!BIG) {
+        const unsigned char *b = reinterpret_cast<const unsigned char *>(sL);
+        v0 = *reinterpret_cast<const int64_t *>(b + (w & 0xfff8u));
+        v1 = *reinterpret_cast<const int64_t *>(b + (w >> 16));
+    } else {
+        const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
+        v0 = sL[c0 & (kLtabSmem - 1)];
+        v1 = sL[c1 & (kLtabSmem - 1)];
+        if (c0 >= (uint32_t)kLtabSmem) v0 = gL[c0];
+        if (c1 >= (uint32_t)kLtabSmem) v1 = gL[c1];
+    }
 }
 
 // S2 + S3 for one point and the R trials of this thread (DESIGN.md section 3; PAPER.md:100 Eq. 3, :106).
@@ -324,7 +334,7 @@ __device__ __forceinline__ int64_t ltab_at(const int64_t *__restrict__ sL, const
 template <int R, bool SHARE_P, bool PZ>
 __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
                                              const double nphi_d, const uint32_t negn, const uint32_t rs,
-                                             const uint32_t (&hb)[(R + 1) / 2]) {
+                                             const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0, const uint32_t inc1) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
 #pragma unroll
@@ -335,7 +345,7 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
         const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
         const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
         const uint32_t j = Iy + Ix * negn;
-        red_add_u32(j * rs + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
+        red_add_u32(j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
     }
 }
 
@@ -346,34 +356,36 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
 template <int R, bool SHARE_P, bool PZ>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
-                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2]) {
+                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0,
+                                           const uint32_t inc1) {
     if (ke - kk >= 4) {
         double2 a0 = sp[kk], a1 = sp[kk + 1];
         do {
             const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, rs, hb);
-            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, rs, hb);
+            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
             a0 = sp[kk + 4];
             a1 = sp[kk + 5];
-            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, rs, hb);
-            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, rs, hb);
+            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
             kk += 4;
         } while (ke - kk >= 4);
     }
-    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, rs, hb);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
 }
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
 template <int R, bool SHARE_P>
 __device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ sp, int kk, const int ke,
                                                    const double (&invP)[R], const double (&cc)[R], const int n_phi,
-                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2]) {
+                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2],
+                                                   const uint32_t inc0, const uint32_t inc1) {
     for (; kk < ke; ++kk) {
         const double2 p = sp[kk];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
-            red_add_u32((uint32_t)j * rs + hb[r >> 1], (r & 1) ? 0x10000u : 1u);
+            red_add_u32((uint32_t)j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
         }
     }
 }
@@ -387,13 +399,15 @@ __device__ __forceinline__ uint32_t fetch_word(const int j, const int n_phi, con
 }
 
 template <int R, bool DUMP, bool BIG>
-__device__ __forceinline__ void close_word(const uint32_t w, const int j, const int w2, const int n_phi,
+__device__ __forceinline__ void close_word(const uint32_t w, const int j, const int w2, const int n_phi, const uint32_t us,
                                            int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
                                            const int lc, const int64_t s0, const bool (&valid)[R], const int seg_i) {
-    const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-    S2[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
-    if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
+    int64_t v0, v1;
+    ltab_pair<BIG>(sL, prm.ltab, w, us, v0, v1);
+    S2[2 * w2] += v0;
+    if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
     if (DUMP) {
+        const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
         if (valid[2 * w2])
             prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
         if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
@@ -409,7 +423,7 @@ __device__ __forceinline__ void close_word(const uint32_t w, const int j, const 
 // the looked-up count is w[k] + w[k-1] (packed 16-bit pairs; needs 2N <= 65535); the folds and the plain marginal are
 // unchanged, the overlap costs one add per word.
 template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL>
-__device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off,
+__device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off, const uint32_t us,
                                               const uint32_t (&hb)[(R + 1) / 2],
                                               uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
                                               const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
@@ -433,10 +447,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
                     const uint32_t ww = w[jj][w2];
                     if (REGM) mg[REGM ? j0 + jj : 0][w2] += ww;
                     else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, ww);
-                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
                     else {
                         if (j0 + jj == 0) first[w2] = ww;
-                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
                         prev[w2] = ww;
                     }
                 }
@@ -447,10 +461,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
             for (int w2 = 0; w2 < RW; ++w2) {
                 const uint32_t ww = fetch_word(j, n_phi, rs, hb[w2]);
                 red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, ww);
-                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
                 else {
                     if (j == 0) first[w2] = ww;
-                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
                     prev[w2] = ww;
                 }
             }
@@ -459,7 +473,7 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
     if (OVL) {  // bin 0 = cells n_phi-1 and 0
 #pragma unroll
         for (int w2 = 0; w2 < RW; ++w2)
-            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, S2, sL, prm, lc, s0, valid, seg_i);
+            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
     }
 }
 
@@ -479,9 +493,9 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     const int n_phi = NPHI > 0 ? NPHI : prm.n_phi, n_m = prm.n_m;
     const uint32_t rs = (uint32_t)NT * 4u;  // bytes between the counter rows of consecutive phase bins
 
-    // shared-memory carve-up: the L table first (compile-time offset, so lookups are LDS.64 [c*8 + imm]), points last
-    int64_t *sL = reinterpret_cast<int64_t *>(smem_raw);                         // [kLtabSmem]
-    uint64_t *full = reinterpret_cast<uint64_t *>(sL + kLtabSmem);               // [2]
+    // shared-memory carve-up (dynamic part; the L table is static so that lookups are LDS.64 [offset + const]), points last
+    __shared__ __align__(16) int64_t sL[kLtabSmem];  // static: its shared address is a link-time constant
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);                     // [2]
     int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
     uint64_t *sstat = reinterpret_cast<uint64_t *>(sseg + GCE_CE_MAX_BINS + 4);  // [kMaxWarps][kStatWords]
     uint32_t *hist = reinterpret_cast<uint32_t *>(sstat + kMaxWarps * kStatWords); // [RW][n_phi + 1][NT], 16-byte aligned
@@ -540,6 +554,8 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     for (int w2 = 0; w2 < RW; ++w2) hb[w2] = smem_u32(hist) + (uint32_t)tid * 4u + (uint32_t)w2 * plane;
     const bool ovl = !DUMP && prm.overlap != 0;  // N2: 2N table entries per trial
     const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)(ovl ? 2 * N : N) : 0.0;
+    const uint32_t us = ((ovl ? 2 : 1) * N <= 8191) ? 3u : 0u;  // counter unit 2^us: a field is its table entry's byte offset
+    const uint32_t inc0 = 1u << us, inc1 = 0x10000u << us;
     uint32_t mg[NPHI_REG][RW];  // phase marginal n_j of the R trials (NPHI > 0), packed like the histogram
 #pragma unroll
     for (int j = 0; j < NPHI_REG; ++j)
@@ -602,10 +618,10 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb);
-                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb);
+                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
                     } else {
-                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb);
+                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, inc0, inc1);
                     }
                 }
                 if (b1 > k_end) break;  // the bin continues in the next buffer
@@ -613,15 +629,15 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 if (b1 > b0) {
                     // a cell of this bin holds at most b1 - b0 points (twice that with overlapping bins)
                     if (!ovl) {
-                        if (b1 - b0 < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, DUMP, false, false>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        if (us == 3u && b1 - b0 < kLtabSmem)
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, DUMP, true, false>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                     } else if (!DUMP) {
-                        if (2 * (b1 - b0) < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, false, false, true>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        if (us == 3u && 2 * (b1 - b0) < kLtabSmem)
+                            close_mag_bin<NPHI, REGM, R, false, false, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, false, true, true>(n_phi, rs, marg_off, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, false, true, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                     }
                 }
                 ++seg_s;
@@ -639,10 +655,10 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
         for (int r = 0; r < R; ++r) S1[r] = 0;
         if (N > 0) {
             auto add_marg = [&](const uint32_t w, const int w2, auto big) {
-                constexpr bool BIG = decltype(big)::value;
-                const uint32_t c0 = w & 0xffffu, c1 = w >> 16;
-                S1[2 * w2] += ltab_at<BIG>(sL, prm.ltab, c0);
-                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += ltab_at<BIG>(sL, prm.ltab, c1);
+                int64_t v0, v1;
+                ltab_pair<decltype(big)::value>(sL, prm.ltab, w, us, v0, v1);
+                S1[2 * w2] += v0;
+                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
             };
             auto marg_pass = [&](auto big, auto ovlt) {
                 constexpr bool OVL = decltype(ovlt)::value;
@@ -671,8 +687,8 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                     for (int w2 = 0; w2 < RW; ++w2) add_marg(first[w2] + prev[w2], w2, big);
                 }
             };
-            if (!ovl) { if (N < kLtabSmem) marg_pass(FalseT{}, FalseT{}); else marg_pass(TrueT{}, FalseT{}); }
-            else { if (2 * N < kLtabSmem) marg_pass(FalseT{}, TrueT{}); else marg_pass(TrueT{}, TrueT{}); }
+            if (!ovl) { if (us == 3u && N < kLtabSmem) marg_pass(FalseT{}, FalseT{}); else marg_pass(TrueT{}, FalseT{}); }
+            else { if (us == 3u && 2 * N < kLtabSmem) marg_pass(FalseT{}, TrueT{}); else marg_pass(TrueT{}, TrueT{}); }
         }
         double ce[R];
         int64_t S[R];
@@ -892,7 +908,7 @@ constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-m
 constexpr int kMinPoints = 640;           // smallest point buffer; also the top-k merge scratch (16 B x 20 warps x 32)
 
 size_t search_smem_fixed() {
-    return sizeof(int64_t) * kLtabSmem + sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) +
+    return sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) +
            sizeof(uint64_t) * kMaxWarps * kStatWords;
 }
 // counter rows of one thread: histogram (n_phi + 1 rows, the last one catches RN(x * n_phi) == n_phi * (floor(x) + 1)),
