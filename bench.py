@@ -339,6 +339,54 @@ def run_ours(args):
     return 0
 
 
+# ----------------------------------------------------------------------------------------- Fig. 3 sweep
+def run_sweep(args):
+    """The paper's only timing result (Fig. 3): time per light curve per search point against the
+    number of search points, for light curves of 100 / 1000 points and 15 plain / 50 overlapping phase bins.  Prints
+    one JSON line per grid size and a markdown table on stderr; fused argmin + Eq. 5 statistics, no cube."""
+    import torch
+    from paper_2006_06866_b200.build import build
+    build()
+    import paper_2006_06866_b200 as gce
+    dev = torch.device("cuda", 0)
+    rows = []
+    for n_obs in (100, 1000):
+        for n_phi, ovl in ((15, False), (50, True)):
+            for sp in (10 ** 3, 10 ** 4, 10 ** 5, 10 ** 6, 10 ** 7, 10 ** 8):
+                w = W.fig3_batch(n_obs, sp, n_phi)
+                d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+                t_, m_, o_, p_, pd_ = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
+                prm = gce.make_params(n_phi, 10, top_k=1, want_stats=True, overlap=ovl)
+                bidx = torch.empty((w.n_lc, 1), dtype=torch.int64, device=dev)
+                bce = torch.empty((w.n_lc, 1), dtype=torch.float32, device=dev)
+                st = torch.empty((w.n_lc, 4), dtype=torch.float64, device=dev)
+                ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, w.n_p, w.n_pdot, prm),
+                                 dtype=torch.uint8, device=dev)
+                reps = 3 if sp >= 10 ** 7 else 10
+                for _ in range(3):
+                    gce.gce_ce_search(t_, m_, o_, p_, pd_, prm, None, bidx, bce, st, ws)
+                torch.cuda.synchronize()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                for _ in range(reps):
+                    gce.gce_ce_search(t_, m_, o_, p_, pd_, prm, None, bidx, bce, st, ws)
+                b.record()
+                b.synchronize()
+                ms = a.elapsed_time(b) / reps
+                trials = w.n_p * w.n_pdot
+                row = {"sweep": "fig3", "n_obs": n_obs, "n_phase_bins": n_phi, "overlap": ovl, "n_lc": w.n_lc,
+                       "search_points": trials, "ms": ms, "ns_per_lc_per_search_point": ms * 1e6 / (w.n_lc * trials),
+                       "point_folds_per_s": w.point_folds / (ms * 1e-3)}
+                rows.append(row)
+                print(json.dumps(row), flush=True)
+    print("| N_obs | phase bins | search points / LC | ms (16 LCs) | ns per LC per search point | point-folds/s |", file=sys.stderr)
+    print("|---|---|---|---|---|---|", file=sys.stderr)
+    for r in rows:
+        print(f"| {r['n_obs']} | {r['n_phase_bins']}{' overlapping' if r['overlap'] else ''} | {r['search_points']:.0e} | "
+              f"{r['ms']:.3f} | {r['ns_per_lc_per_search_point']:.3f} | {r['point_folds_per_s']:.3e} |", file=sys.stderr)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -351,9 +399,12 @@ def main():
     ap.add_argument("--n-phase-bins", type=int, default=0, help="override the config's phase bin count (named in config)")
     ap.add_argument("--n-mag-bins", type=int, default=0, help="override the config's magnitude bin count")
     ap.add_argument("--overlap", action="store_true", help="50 %% overlapping phase bins (N2, PAPER.md:106)")
+    ap.add_argument("--sweep", action="store_true", help="the paper's Fig. 3 sweep instead of the benchmark line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     OVERLAP[0] = bool(args.overlap)
+    if args.sweep:
+        return run_sweep(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

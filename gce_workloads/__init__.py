@@ -223,6 +223,19 @@ def config_c5(n_lc=16, n_p=1 << 17, n_pdot=256, seed=4) -> Workload:
                     30, 10, top_k=16, want_cube=False, truth=truth)
 
 
+def fig3_batch(n_obs, n_search_points, n_phase_bins, n_lc=16, n_pdot=32, seed=7) -> Workload:
+    """Workload of the paper's timing figure (Fig. 3): light curves of n_obs points (100 or 1000)
+    over ten years (VRO-like, :90), a grid of n_search_points = n_p x n_pdot trials per light curve (the paper searches
+    groups of 32 / 128 / 512 Pdot values, :158), 15 or 50 phase bins x 10 magnitude bins.  Two-dip model as C4."""
+    n_p = max(1, int(round(n_search_points / n_pdot)))
+    lcs, truth = _two_dip_batch(seed, n_lc, lambda r: lsst_like_cadence(r, n_obs), 600.0, 7200.0, (-12.0, -10.0),
+                                (0.05, 0.5), (0.05, 0.5), 0.08)
+    times, mags, offs = _pack(lcs)
+    return Workload(f"fig3-N{n_obs}-phi{n_phase_bins}", times, mags, offs, _freq_grid(1 / 14400.0, 1 / 300.0, n_p),
+                    np.ascontiguousarray(np.linspace(-1e-10, 0.0, int(n_pdot))), n_phase_bins, 10, top_k=1,
+                    want_cube=False, truth=truth)
+
+
 CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5}
 
 
