@@ -112,10 +112,11 @@ def make_workload(name, rank, shrink):
     kw = {}
     if shrink:  # --quick: same ranges, smaller grid (for smoke-testing the bench itself; never a reported number)
         kw = {"C1": {}, "C2": dict(n_lc=8, n_p=2000), "C3": dict(n_lc=4, n_p=2000, n_pdot=64),
-              "C4": dict(n_lc=16, n_p=4000), "C5": dict(n_lc=2, n_p=512, n_pdot=32)}[name]
+              "C4": dict(n_lc=16, n_p=4000), "C5": dict(n_lc=2, n_p=512, n_pdot=32),
+              "P1": dict(n_lc=4, n_p=20000, n_pdot=32)}[name]
     if rank > 0:
         # weak scaling: every rank owns a batch of the same shape; rank r re-draws it from seed + 1000 r
-        kw = dict(kw, seed={"C1": 0, "C2": 1, "C3": 2, "C4": 3, "C5": 4}[name] + 1000 * rank)
+        kw = dict(kw, seed={"C1": 0, "C2": 1, "C3": 2, "C4": 3, "C5": 4, "P1": 9}[name] + 1000 * rank)
     return W.make(name, **kw)
 
 
@@ -168,6 +169,9 @@ def run_reference(args):
     if rank != 0:
         return 0
     import oracle
+    if args.config == "P1":
+        args.overlap = True
+        OVERLAP[0] = True
     w = apply_binning(make_workload(args.config, 0, args.quick), args)
     per_step = max(1.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
     sample, desc = oracle_sample(w, per_step)
@@ -188,7 +192,9 @@ def run_reference(args):
 
 
 def workload_config(w, args):
-    return {"workload": f"{w.name} (BASELINE.json:configs[{int(w.name[1]) - 1}])" + (" QUICK-SHRUNK" if args.quick else ""),
+    src = (f"BASELINE.json:configs[{int(w.name[1]) - 1}]" if w.name[0] == "C" else
+           "the paper's production grid, PAPER.md:166-170, 50 overlapping phase bins; not a BASELINE.json config")
+    return {"workload": f"{w.name} ({src})" + (" QUICK-SHRUNK" if args.quick else ""),
             "n_lc": w.n_lc, "n_obs_total": w.total_points, "n_p": w.n_p, "n_pdot": w.n_pdot,
             "n_phase_bins": w.n_phase_bins, "n_mag_bins": w.n_mag_bins, "overlap": bool(args.overlap), "top_k": w.top_k, "ce_cube": bool(w.want_cube),
             "point_folds_per_step_per_gpu": w.point_folds, "parallelism": f"independent light-curve batches x{args.gpus}",
@@ -218,6 +224,9 @@ def run_ours(args):
         dist.barrier()
     import paper_2006_06866_b200 as gce
 
+    if args.config == "P1":
+        args.overlap = True   # the paper's production binning
+        OVERLAP[0] = True
     w = apply_binning(make_workload(args.config, rank, args.quick), args)
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     times, mags, offs, periods, pdots = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
@@ -392,7 +401,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5", "P1"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true", help="shrunk grid, to test the bench itself; not a reportable number")
     ap.add_argument("--no-cpu-baseline", action="store_true")

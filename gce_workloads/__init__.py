@@ -236,7 +236,30 @@ def fig3_batch(n_obs, n_search_points, n_phase_bins, n_lc=16, n_pdot=32, seed=7)
                     want_cube=False, truth=truth)
 
 
-CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5}
+def vro_like_cadence(rng, n_obs: int, mean_dt_days=7.0, sigma_dt_days=1.0) -> np.ndarray:
+    """"The time difference between each observation point is sampled from a Gaussian distribution with
+    mean dt" -- VRO-like: ten-year baseline, about 7 days between observations, n ~ 500.  (The width of the Gaussian is
+    not given; one day is this harness's choice.)"""
+    dt = np.maximum(rng.normal(mean_dt_days, sigma_dt_days, size=n_obs), 0.01) * DAY
+    t = np.cumsum(dt)
+    return t - t[0]
+
+
+def config_paper(n_lc=100, n_p=5_183_995, n_pdot=32, seed=9) -> Workload:
+    """NEXT item N4 -- the paper's production search: 5,183,995 frequencies linearly spaced
+    from 2/B (B = 10 yr) to 1/(3 min), 32 / 128 / 512 Pdot values log-spaced from -1e-12 to -1e-10, 100 light curves of
+    about 500 points, 50 overlapping phase bins x 10 magnitude bins.  The cube (1.7e10 values at 32 Pdots) is never
+    materialised: fused top-k + Eq. 5 statistics.  Synthetic two-dip light curves stand in for the COSMIC / ellc set."""
+    lcs, truth = _two_dip_batch(seed, n_lc, lambda r: vro_like_cadence(r, 500), 300.0, 3600.0, (-12.0, -10.3),
+                                (0.1, 0.8), (0.05, 0.4), 0.2)
+    times, mags, offs = _pack(lcs)
+    B = 10.0 * 365.25 * DAY
+    pdots = -np.logspace(-12.0, -10.0, int(n_pdot))
+    return Workload("P1", times, mags, offs, _freq_grid(2.0 / B, 1.0 / 180.0, n_p), np.ascontiguousarray(pdots),
+                    50, 10, top_k=5, want_cube=False, truth=truth)
+
+
+CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5, "P1": config_paper}
 
 
 def make(name: str, **kw) -> Workload:

@@ -97,6 +97,39 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
                        const gce_ce_params *prm_host, void *out_ce, int64_t *out_best_idx,
                        float *out_best_ce, double *out_stats);
 
+/*
+ * Period sub-ranges and exact merging (NEXT item N4; "batching over light curves / Pdots" with the
+ * per-batch minima merged afterwards; SURVEY.md section 8e period-axis split across GPUs).
+ *
+ * gce_ce_search_partial searches the periods [ip_begin, ip_end) of the grid for every light curve and writes, instead
+ * of the final selection, one PARTIAL blob per light curve:
+ *   out_partial   int64[n_lc][gce_ce_partial_words(top_k)] =
+ *                 { S[top_k] ascending, q[top_k], 8 words of Eq. 5 sums, N, pivot }
+ *                 with S = N * CE * 2^42 as an exact integer (INT64_MAX where fewer than top_k trials exist) and q the
+ *                 flat index in the WHOLE grid (ip * n_pdot + ipd); the Eq. 5 words are filled when want_stats = 1.
+ *   out_ce        NULL, or the cube slice [n_lc][ip_end - ip_begin][n_pdot]
+ *   periods       the whole grid double[n_p]; workspace as for gce_ce_workspace_bytes(total_points, n_lc,
+ *                 ip_end - ip_begin, n_pdot, prm)
+ * gce_ce_merge_partials merges n_parts such blob arrays, int64[n_parts][n_lc][words] (disjoint period ranges of the same
+ * light curves and the same prm; device memory, e.g. gathered from other batches or GPUs), into out_best_idx /
+ * out_best_ce / out_stats exactly as gce_ce_search would have written them for the union of the ranges: all keys and
+ * sums are integers, so the result is bit-identical however the grid was split.
+ */
+size_t gce_ce_partial_words(int32_t top_k);
+
+int gce_ce_search_partial(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                          int64_t total_points, const double *periods, int64_t n_p, const double *pdots,
+                          int64_t n_pdot, const gce_ce_params *prm_host, int64_t ip_begin, int64_t ip_end,
+                          void *out_ce, int64_t *out_partial, void *workspace, size_t workspace_bytes, void *stream);
+
+int gce_ce_merge_partials(const int64_t *partials, int32_t n_parts, int32_t n_lc, const gce_ce_params *prm_host,
+                          int64_t *out_best_idx, float *out_best_ce, double *out_stats, void *stream);
+
+/* Same merge, but the result is again one partial blob array int64[n_lc][words] (hierarchical merging: the chunks of
+ * one GPU first, then one blob array per GPU over the interconnect). */
+int gce_ce_merge_partials_to_partial(const int64_t *partials, int32_t n_parts, int32_t n_lc,
+                                     const gce_ce_params *prm_host, int64_t *out_partial, void *stream);
+
 /* Test-only: the production search kernel run in "dump" mode over a list of flat trial indices
  * (device int64[n_trials], the same list for every light curve); writes the histogram counts
  *   out_counts uint32[n_lc][n_trials][n_phase_bins][n_mag_bins]      (phase-major, as Eq. 4's n_ij)

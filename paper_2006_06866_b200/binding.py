@@ -39,18 +39,27 @@ _lib.gce_ce_debug_histogram.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _v
                                         _vp, _i64, _vp, _vp, _vp, _sz, _vp]
 _lib.gce_ce_debug_bins.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _i32, _i64,
                                    _vp, _vp, _vp]
+_lib.gce_ce_partial_words.argtypes = [_i32]
+_lib.gce_ce_partial_words.restype = _sz
+_lib.gce_ce_search_partial.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params), _i64, _i64,
+                                       _vp, _vp, _vp, _sz, _vp]
+_lib.gce_ce_merge_partials.argtypes = [_vp, _i32, _i32, C.POINTER(Params), _vp, _vp, _vp, _vp]
+_lib.gce_ce_merge_partials_to_partial.argtypes = [_vp, _i32, _i32, C.POINTER(Params), _vp, _vp]
+_lib.gce_ce_merge_partials_to_partial.restype = C.c_int
 _lib.gce_ce_validate_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params)]
 _lib.gce_ce_launch_count.argtypes = [_i32, C.POINTER(Params)]
 _lib.gce_ce_strerror.argtypes = [C.c_int]
 _lib.gce_ce_strerror.restype = C.c_char_p
 _lib.gce_ce_version.restype = C.c_char_p
 for _f in ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
-           "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_last_cuda_error"):
+           "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_last_cuda_error",
+           "gce_ce_search_partial", "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial"):
     getattr(_lib, _f).restype = C.c_int
 
 EXPORTS = ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
            "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_strerror",
-           "gce_ce_last_cuda_error", "gce_ce_version")
+           "gce_ce_last_cuda_error", "gce_ce_version", "gce_ce_partial_words", "gce_ce_search_partial",
+           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial")
 
 
 class GceError(RuntimeError):
@@ -137,6 +146,48 @@ def gce_ce_search(times, mags, lc_offsets, periods, pdots, prm: Params, out_ce=N
                               periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), _ptr(out_ce),
                               _ptr(out_best_idx), _ptr(out_best_ce), _ptr(out_stats), _ptr(workspace),
                               workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def gce_ce_partial_words(top_k) -> int:
+    return int(_lib.gce_ce_partial_words(int(top_k)))
+
+
+def gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm: Params, ip_begin, ip_end, out_partial,
+                          out_ce=None, workspace=None, stream=None):
+    """Search the periods [ip_begin, ip_end) of the grid; out_partial int64 [n_lc][gce_ce_partial_words(top_k)]."""
+    times, mags = _dev(times, torch.float64), _dev(mags, torch.float64)
+    lc_offsets = _dev(lc_offsets, torch.int64)
+    periods, pdots = _dev(periods, torch.float64), _dev(pdots, torch.float64)
+    n_lc = lc_offsets.numel() - 1
+    _dev(out_partial, torch.int64)
+    if out_partial.numel() != n_lc * gce_ce_partial_words(prm.top_k):
+        raise ValueError("out_partial has the wrong number of elements")
+    if out_ce is not None:
+        _dev(out_ce, torch.float64 if prm.ce_fp64 else torch.float32)
+        if out_ce.numel() != n_lc * (int(ip_end) - int(ip_begin)) * pdots.numel():
+            raise ValueError("out_ce has the wrong number of elements")
+    if workspace is None or not workspace.is_cuda:
+        raise TypeError("workspace must be a CUDA tensor (see gce_ce_workspace_bytes)")
+    _check(_lib.gce_ce_search_partial(_ptr(times), _ptr(mags), _ptr(lc_offsets), n_lc, times.numel(), _ptr(periods),
+                                      periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), int(ip_begin),
+                                      int(ip_end), _ptr(out_ce), _ptr(out_partial), _ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def gce_ce_merge_partials(partials, n_parts, n_lc, prm: Params, out_best_idx=None, out_best_ce=None, out_stats=None,
+                          stream=None):
+    """Merge int64 [n_parts][n_lc][words] partial blobs into the final selection / Eq. 5 statistics."""
+    _dev(partials, torch.int64)
+    if partials.numel() != int(n_parts) * int(n_lc) * gce_ce_partial_words(prm.top_k):
+        raise ValueError("partials has the wrong number of elements")
+    if out_best_idx is not None:
+        _dev(out_best_idx, torch.int64)
+    if out_best_ce is not None:
+        _dev(out_best_ce, torch.float32)
+    if out_stats is not None:
+        _dev(out_stats, torch.float64)
+    _check(_lib.gce_ce_merge_partials(_ptr(partials), int(n_parts), int(n_lc), C.byref(prm), _ptr(out_best_idx),
+                                      _ptr(out_best_ce), _ptr(out_stats), _stream(stream)))
 
 
 def gce_ce_debug_histogram(times, mags, lc_offsets, periods, pdots, prm: Params, trial_q, out_counts, out_ce_at=None,
@@ -236,3 +287,53 @@ def search(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, to
         workspace = torch.empty(nbytes, dtype=torch.uint8, device=dev)
     gce_ce_search(times, mags, lc_offsets, periods, pdots, prm, ce, bidx, bce, stats, workspace, stream)
     return SearchResult(ce, bidx, bce, stats)
+
+
+def search_period_chunks(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, chunks, top_k=1,
+                         want_stats=True, overlap=False, ce_fp64=False, cube_sink=None, dist=None, stream=None) -> SearchResult:
+    """The search over a list of period ranges [(ip_begin, ip_end), ...] -- this process's share of the grid -- merged
+    exactly (batches bound the memory, their minima are merged; period-axis split when
+    there are fewer light curves than GPUs).  One workspace and one partial buffer are reused for every chunk.
+    cube_sink(ip_begin, ip_end, ce_slice) receives each cube slice [n_lc][ip_end - ip_begin][n_pdot] (device tensor,
+    overwritten by the next chunk) when given.  With `dist` (initialised torch.distributed, NCCL) the partial blobs of
+    all ranks are all-gathered -- n_lc x (2 top_k + 10) int64 per rank, the only exchange of the path -- and every rank
+    merges them, so every rank returns the whole grid's selection.  Argument marshalling and plumbing only: the merge
+    runs in the library's kernels."""
+    prm = make_params(n_phase_bins, n_mag_bins, top_k, ce_fp64, want_stats, overlap)
+    dev = times.device
+    n_lc = lc_offsets.numel() - 1
+    n_pdot = pdots.numel()
+    words = gce_ce_partial_words(top_k)
+    chunks = [(int(a), int(b)) for a, b in chunks]
+    widest = max([b - a for a, b in chunks], default=0)
+    ws = torch.empty(gce_ce_workspace_bytes(times.numel(), n_lc, widest, n_pdot, prm), dtype=torch.uint8, device=dev)
+    parts = torch.empty((max(len(chunks), 1), n_lc, words), dtype=torch.int64, device=dev)
+    ce = None
+    if cube_sink is not None and widest > 0:
+        ce = torch.empty(n_lc * widest * n_pdot, dtype=torch.float64 if ce_fp64 else torch.float32, device=dev)
+    if not chunks:  # a rank with no periods still contributes a (neutral) blob
+        gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm, 0, 0, parts[0], None, ws, stream)
+    for i, (a, b) in enumerate(chunks):
+        sl = ce[: n_lc * (b - a) * n_pdot] if ce is not None else None
+        gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm, a, b, parts[i], sl, ws, stream)
+        if cube_sink is not None:
+            cube_sink(a, b, sl.view(n_lc, b - a, n_pdot))
+    n_parts = parts.shape[0]
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        # ranks may hold different numbers of chunks: merge locally first, then exchange one blob array per rank
+        local = torch.empty((1, n_lc, words), dtype=torch.int64, device=dev)
+        _merge_to_partial(parts, n_parts, n_lc, prm, local, stream)
+        gathered = [torch.empty_like(local) for _ in range(dist.get_world_size())]
+        dist.all_gather(gathered, local)
+        parts = torch.cat(gathered, dim=0)
+        n_parts = parts.shape[0]
+    bidx = torch.empty((n_lc, top_k), dtype=torch.int64, device=dev) if top_k > 0 else None
+    bce = torch.empty((n_lc, top_k), dtype=torch.float32, device=dev) if top_k > 0 else None
+    stats = torch.empty((n_lc, 4), dtype=torch.float64, device=dev) if want_stats else None
+    gce_ce_merge_partials(parts, n_parts, n_lc, prm, bidx, bce, stats, stream)
+    return SearchResult(None, bidx, bce, stats)
+
+
+def _merge_to_partial(parts, n_parts, n_lc, prm, out_partial, stream=None):
+    _check(_lib.gce_ce_merge_partials_to_partial(_ptr(parts), int(n_parts), int(n_lc), C.byref(prm), _ptr(out_partial),
+                                                 _stream(stream)))

@@ -67,6 +67,7 @@ struct SearchParams {
     const double *pdots;
     const int64_t *trial_q;    // DUMP only
     int64_t n_p, n_pdot, n_trials;
+    int64_t q_off;             // flat index of this call's first trial in the caller's grid (period sub-range)
     int64_t tiles_per_lc;
     int32_t jobs_per_lc;
     int32_t n_phi, n_m;
@@ -585,7 +586,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
             valid[r] = s < prm.n_trials;
             int64_t q = 0;
             if (valid[r]) q = DUMP ? prm.trial_q[s] : s;
-            qv[r] = q;
+            qv[r] = q + prm.q_off;  // reported index: flat q of the caller's whole grid
             double ip = 0.0, c = 0.0;
             if (valid[r] && (!SHARE_P || r == 0)) ip = __ddiv_rn(1.0, prm.periods[q / prm.n_pdot]);
             if (SHARE_P && r > 0) ip = invP[0];
@@ -788,47 +789,69 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     }
 }
 
-// One warp per light curve: merge jobs_per_lc x k candidates, write the user-facing selection.
-__global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ part_S, const int64_t *__restrict__ part_q,
-                                                   const LcInfo *__restrict__ info, int jobs_per_lc, int K, int mult,
-                                                   int64_t *__restrict__ out_idx, float *__restrict__ out_ce) {
+// ---- S5 / Eq. 5 merges.  One warp per light curve.  The candidates / partial sums of light curve lc live at
+// base[lc * lc_stride + p * part_stride + ...], p < n_parts: inside one call the parts are the CTAs (jobs) of k_search,
+// in gce_ce_merge_partials they are the caller's partial blobs (period ranges, batches, GPUs).  Keys are
+// the exact integers (S = N*CE*2^42, flat q), so the merged result does not depend on the split.
+// Partial blob of one light curve (int64 words): [0,K) S ascending, [K,2K) q, [2K,2K+8) Eq. 5 sums, [2K+8] N, [2K+9] pivot.
+__host__ __device__ inline int partial_words(int K) { return 2 * K + kStatWords + 2; }
+
+__global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ S, const int64_t *__restrict__ q,
+                                                   int64_t lc_stride, int64_t part_stride, int n_parts, int K,
+                                                   const LcInfo *__restrict__ info, const int64_t *__restrict__ npts,
+                                                   int64_t npts_stride, int mult, int64_t *__restrict__ out_idx,
+                                                   float *__restrict__ out_ce, int64_t *__restrict__ out_raw,
+                                                   int64_t raw_stride) {
     const int lc = blockIdx.x, lane = threadIdx.x;
     WarpTopK top;
     top.reset(K);
-    const int total = jobs_per_lc * K;
+    const int total = n_parts * K;
     for (int e = 0; e < total; e += 32) {
         const int i = e + lane;
-        const int64_t cS = i < total ? part_S[(int64_t)lc * total + i] : kInfS;
-        const int64_t cq = i < total ? part_q[(int64_t)lc * total + i] : kInfS;
-        top.offer(cS, cq);
+        const int64_t at = (int64_t)lc * lc_stride + (int64_t)(i / K) * part_stride + (i % K);
+        top.offer(i < total ? S[at] : kInfS, i < total ? q[at] : kInfS);
     }
-    if (lane < K) {
-        const bool have = top.S != kInfS;
-        const int n = info[lc].n;
-        out_idx[(int64_t)lc * K + lane] = have ? top.q : -1;
-        if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)(mult * n))) : CUDART_NAN_F;
+    if (lane >= K) return;
+    if (out_raw) {  // partial blob: exact keys, kInfS where fewer than K trials exist
+        out_raw[(int64_t)lc * raw_stride + lane] = top.S;
+        out_raw[(int64_t)lc * raw_stride + K + lane] = top.q;
+        return;
     }
+    const bool have = top.S != kInfS;
+    const int64_t n = info ? (int64_t)info[lc].n : npts[(int64_t)lc * npts_stride];
+    out_idx[(int64_t)lc * K + lane] = have ? top.q : -1;
+    if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)(mult * n))) : CUDART_NAN_F;
 }
 
-// Eq. 5: one warp per light curve sums the per-CTA partials (exact integers, so the result does not
-// depend on how the trials were split over CTAs, batches or GPUs) and converts once to fp64:
-// out_stats[lc] = {mean CE, population std, min CE, rho = (mean - min) / std}.
+// Eq. 5: sums the partials (exact integers) and converts once to fp64:
+// out_stats[lc] = {mean CE, population std, min CE, rho = (mean - min) / std}; or writes the raw sums to a partial blob.
 __device__ __forceinline__ double u128_to_double(u128_t v) {
     return (double)(uint64_t)(v >> 64) * 18446744073709551616.0 + (double)(uint64_t)v;
 }
-__global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__ part, const LcInfo *__restrict__ info,
-                                                    int jobs_per_lc, int mult, double *__restrict__ out_stats) {
+__global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__ part, int64_t lc_stride, int64_t part_stride,
+                                                    int n_parts, const LcInfo *__restrict__ info,
+                                                    const int64_t *__restrict__ npts, int64_t npts_stride, int mult,
+                                                    double *__restrict__ out_stats, int64_t *__restrict__ out_raw,
+                                                    int64_t raw_stride) {
     __shared__ uint64_t sh[32][kStatWords];
     const int lc = blockIdx.x, lane = threadIdx.x;
     uint64_t acc[kStatWords];
     stat_init(acc);
-    for (int j = lane; j < jobs_per_lc; j += 32) stat_merge(acc, part + ((int64_t)lc * jobs_per_lc + j) * kStatWords);
+    for (int j = lane; j < n_parts; j += 32) stat_merge(acc, part + (int64_t)lc * lc_stride + (int64_t)j * part_stride);
     for (int i = 0; i < kStatWords; ++i) sh[lane][i] = acc[i];
     __syncwarp();
     if (lane != 0) return;
     for (int l = 1; l < 32; ++l) stat_merge(acc, sh[l]);
+    const int64_t n_pts = info ? (int64_t)info[lc].n : npts[(int64_t)lc * npts_stride];
+    const int64_t pivot = info ? info[lc].K : npts[(int64_t)lc * npts_stride + 1];
+    if (out_raw) {
+        int64_t *o = out_raw + (int64_t)lc * raw_stride;
+        for (int i = 0; i < kStatWords; ++i) o[i] = (int64_t)acc[i];
+        o[kStatWords] = n_pts;
+        o[kStatWords + 1] = pivot;
+        return;
+    }
     double *o = out_stats + (int64_t)lc * 4;
-    const int n_pts = info[lc].n;
     if (acc[0] == 0 || n_pts <= 0) { o[0] = o[1] = o[2] = o[3] = CUDART_NAN; return; }
     const double n = (double)acc[0];
     const u128_t A = ((u128_t)acc[2] << 64) | acc[1];
@@ -839,7 +862,7 @@ __global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__
     const double mean_d = sum_d / n;
     double var = sum_d2 / n - mean_d * mean_d;
     if (var < 0.0 || acc[6] == acc[7]) var = 0.0;  // min == max: every trial has the same CE, the spread is exactly 0
-    const double mean = ((double)info[lc].K + mean_d) * scale;
+    const double mean = ((double)pivot + mean_d) * scale;
     const double sd = sqrt(var) * scale;
     const double mn = (double)(int64_t)acc[6] * scale;
     o[0] = mean; o[1] = sd; o[2] = mn; o[3] = (mean - mn) / sd;
@@ -1105,8 +1128,9 @@ int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int6
 static int run_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                       int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
                       const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce, double *out_stats,
-                      const int64_t *trial_q, int64_t n_dump, uint32_t *out_counts, double *out_ce_at, void *workspace,
-                      size_t workspace_bytes, void *stream) {
+                      const int64_t *trial_q, int64_t n_dump, uint32_t *out_counts, double *out_ce_at, int64_t ip_begin,
+                      int64_t *out_partial, void *workspace, size_t workspace_bytes, void *stream) {
+    // periods / n_p describe THIS call's period range; ip_begin is its offset in the caller's grid (0 for a whole grid)
     const bool dump = out_counts != nullptr;
     int rc = check_params(prm);
     if (rc) return rc;
@@ -1119,10 +1143,14 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     if (dump) {
         if (!trial_q || n_dump < 0) return GCE_CE_ERR_POINTER;
     } else {
-        if (!out_ce && !out_best_idx && !out_stats) return GCE_CE_ERR_POINTER;
-        if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
-        if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
-        if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+        if (out_partial) {
+            if (out_best_idx || out_best_ce || out_stats) return GCE_CE_ERR_POINTER;
+        } else {
+            if (!out_ce && !out_best_idx && !out_stats) return GCE_CE_ERR_POINTER;
+            if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
+            if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
+            if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+        }
     }
     const int64_t n_trials = dump ? n_dump : n_p * n_pdot;
     gce_ce_params lay_prm = *prm;
@@ -1152,6 +1180,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.pts = pts; sp.seg = seg; sp.info = info; sp.lc_offsets = lc_offsets; sp.ltab = ltab;
     sp.periods = periods; sp.pdots = pdots; sp.trial_q = trial_q;
     sp.n_p = n_p; sp.n_pdot = n_pdot; sp.n_trials = n_trials;
+    sp.q_off = dump ? 0 : ip_begin * n_pdot;
     sp.jobs_per_lc = plan.jobs_per_lc;
     sp.tiles_per_lc = plan.tiles_per_lc;
     sp.cap_points = plan.cap_points;
@@ -1178,14 +1207,19 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
         e = cudaEventRecord(reinterpret_cast<cudaEvent_t>(prm->ev_search_end), st);
         if (e != cudaSuccess) return cuda_fail(e);
     }
-    if (!dump && prm->top_k > 0) {
-        k_merge_topk<<<n_lc, 32, 0, st>>>(sp.part_S, sp.part_q, info, n_trials > 0 ? plan.jobs_per_lc : 0, prm->top_k, mult,
-                                          out_best_idx, out_best_ce);
+    const int K = prm->top_k;
+    const int n_jobs = n_trials > 0 ? plan.jobs_per_lc : 0;
+    const int W = partial_words(K);
+    if (!dump && K > 0) {
+        k_merge_topk<<<n_lc, 32, 0, st>>>(sp.part_S, sp.part_q, (int64_t)plan.jobs_per_lc * K, K, n_jobs, K, info, nullptr, 0,
+                                          mult, out_best_idx, out_best_ce, out_partial, W);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e);
     }
-    if (!dump && prm->want_stats) {
-        k_merge_stats<<<n_lc, 32, 0, st>>>(sp.part_stats, info, n_trials > 0 ? plan.jobs_per_lc : 0, mult, out_stats);
+    if (!dump && (prm->want_stats || out_partial)) {
+        k_merge_stats<<<n_lc, 32, 0, st>>>(sp.part_stats, (int64_t)plan.jobs_per_lc * kStatWords, kStatWords,
+                                           prm->want_stats ? n_jobs : 0, info, nullptr, 0, mult, out_stats,
+                                           out_partial ? out_partial + 2 * K : nullptr, W);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e);
     }
@@ -1197,7 +1231,71 @@ int gce_ce_search(const double *times, const double *mags, const int64_t *lc_off
                   const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce, double *out_stats,
                   void *workspace, size_t workspace_bytes, void *stream) {
     return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, out_ce,
-                      out_best_idx, out_best_ce, out_stats, nullptr, 0, nullptr, nullptr, workspace, workspace_bytes, stream);
+                      out_best_idx, out_best_ce, out_stats, nullptr, 0, nullptr, nullptr, 0, nullptr, workspace, workspace_bytes, stream);
+}
+
+size_t gce_ce_partial_words(int32_t top_k) { return (size_t)partial_words(top_k < 0 ? 0 : top_k); }
+
+int gce_ce_search_partial(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                          int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                          const gce_ce_params *prm, int64_t ip_begin, int64_t ip_end, void *out_ce, int64_t *out_partial,
+                          void *workspace, size_t workspace_bytes, void *stream) {
+    if (!out_partial) return GCE_CE_ERR_POINTER;
+    if (ip_begin < 0 || ip_end < ip_begin || ip_end > n_p) return GCE_CE_ERR_RANGE;
+    return run_search(times, mags, lc_offsets, n_lc, total_points, periods ? periods + ip_begin : periods, ip_end - ip_begin,
+                      pdots, n_pdot, prm, out_ce, nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, ip_begin,
+                      out_partial, workspace, workspace_bytes, stream);
+}
+
+int gce_ce_merge_partials(const int64_t *partials, int32_t n_parts, int32_t n_lc, const gce_ce_params *prm,
+                          int64_t *out_best_idx, float *out_best_ce, double *out_stats, void *stream) {
+    int rc = check_params(prm);
+    if (rc) return rc;
+    if (n_parts < 1 || n_lc < 0) return GCE_CE_ERR_RANGE;
+    if (!partials) return GCE_CE_ERR_POINTER;
+    if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
+    if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
+    if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+    if (n_lc == 0) return GCE_CE_OK;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int K = prm->top_k, W = partial_words(K), mult = prm->overlap ? 2 : 1;
+    const int64_t *npts = partials + 2 * K + kStatWords;  // N and the pivot, identical in every part
+    if (K > 0) {
+        k_merge_topk<<<n_lc, 32, 0, st>>>(partials, partials + K, W, (int64_t)n_lc * W, n_parts, K, nullptr, npts, W, mult,
+                                          out_best_idx, out_best_ce, nullptr, 0);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    if (prm->want_stats) {
+        k_merge_stats<<<n_lc, 32, 0, st>>>(reinterpret_cast<const uint64_t *>(partials + 2 * K), W, (int64_t)n_lc * W, n_parts,
+                                           nullptr, npts, W, mult, out_stats, nullptr, 0);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return GCE_CE_OK;
+}
+
+int gce_ce_merge_partials_to_partial(const int64_t *partials, int32_t n_parts, int32_t n_lc, const gce_ce_params *prm,
+                                     int64_t *out_partial, void *stream) {
+    int rc = check_params(prm);
+    if (rc) return rc;
+    if (n_parts < 1 || n_lc < 0) return GCE_CE_ERR_RANGE;
+    if (!partials || !out_partial) return GCE_CE_ERR_POINTER;
+    if (n_lc == 0) return GCE_CE_OK;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int K = prm->top_k, W = partial_words(K), mult = prm->overlap ? 2 : 1;
+    const int64_t *npts = partials + 2 * K + kStatWords;
+    if (K > 0) {
+        k_merge_topk<<<n_lc, 32, 0, st>>>(partials, partials + K, W, (int64_t)n_lc * W, n_parts, K, nullptr, npts, W, mult,
+                                          nullptr, nullptr, out_partial, W);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    k_merge_stats<<<n_lc, 32, 0, st>>>(reinterpret_cast<const uint64_t *>(partials + 2 * K), W, (int64_t)n_lc * W, n_parts,
+                                       nullptr, npts, W, mult, nullptr, out_partial + 2 * K, W);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return GCE_CE_OK;
 }
 
 int gce_ce_debug_histogram(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
@@ -1215,7 +1313,7 @@ int gce_ce_debug_histogram(const double *times, const double *mags, const int64_
         if (e != cudaSuccess) return cuda_fail(e);
     }
     return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, nullptr, nullptr,
-                      nullptr, nullptr, trial_q, n_trials, out_counts, out_ce_at, workspace, workspace_bytes, stream);
+                      nullptr, nullptr, trial_q, n_trials, out_counts, out_ce_at, 0, nullptr, workspace, workspace_bytes, stream);
 }
 
 int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,

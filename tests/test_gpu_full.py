@@ -268,6 +268,7 @@ def test_c4_full_stats_sampled_light_curves(gce, oracle):
     ("C4", dict(n_lc=9, n_p=5000), 15, 8, 5),
     ("C5", dict(n_lc=2, n_p=300, n_pdot=16), 30, 10, 16),    # 2 x points per magnitude bin above the shared table
     ("C1", dict(), 1, 10, 1), ("C1", dict(), 2, 10, 1), ("C1", dict(), 64, 64, 2),
+    ("P1", dict(n_lc=2, n_p=2000, n_pdot=32), 50, 10, 5),    # the paper's production grid shape (N4), log-spaced Pdots
 ])
 def test_overlapping_phase_bins_match_oracle(gce, oracle, name, kw, n_phi, n_m, k):
     """overlap = 1 against the oracle's N2 variant (bin k = plain cells k-1 and k, 2N entries): whole fp64 / fp32 cube,
