@@ -340,7 +340,7 @@ def run_ours(args):
             "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(w, args),
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
-                    "api": "gce_ce_search_host (pinned host buffers; cudaMallocAsync + H2D + search + D2H + sync)"},
+                    "api": "gce_ce_search_host (pinned host buffers; allocation + H2D + search in 8 period chunks with the D2H of each cube slice overlapped on a second stream + sync)"},
             "gpu_launches": launches_per_step * args.steps, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:

@@ -1359,6 +1359,89 @@ int gce_ce_validate_host(const double *times, const double *mags, const int64_t 
     return GCE_CE_OK;
 }
 
+// Host-buffer entry with the cube requested and a grid worth splitting: the period axis is cut into chunks searched
+// back to back on one stream (gce_ce_search_partial, exact merge at the end) while a second stream copies each finished
+// cube slice to the caller's buffer, so the device-to-host transfer of the cube overlaps the search of the next chunk.
+static int search_host_pipelined(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                                 int64_t total, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                                 const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                                 double *out_stats, int n_chunks) {
+    const size_t esz = prm->ce_fp64 ? 8 : 4;
+    const int64_t chunk = (n_p + n_chunks - 1) / n_chunks;
+    const size_t k = (size_t)prm->top_k, W = gce_ce_partial_words(prm->top_k);
+    size_t ws_bytes = 0;
+    int rc = gce_ce_workspace_bytes(total, n_lc, chunk, n_pdot, prm, &ws_bytes);
+    if (rc) return rc;
+    cudaStream_t st = nullptr, st2 = nullptr;
+    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaStreamCreateWithFlags(&st2, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { cudaStreamDestroy(st); return cuda_fail(e); }
+    for (int b = 0; b < 2; ++b) {
+        cudaEventCreateWithFlags(&ev_done[b], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&ev_free[b], cudaEventDisableTiming);
+    }
+    void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
+    void *d_sl[2] = {nullptr, nullptr}, *d_part = nullptr, *d_idx = nullptr, *d_bce = nullptr, *d_st = nullptr;
+    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocAsync(p, bytes ? bytes : 16, st); };
+    const size_t slice_bytes = (size_t)n_lc * (size_t)chunk * (size_t)n_pdot * esz;
+    rc = GCE_CE_OK;
+    do {
+        if ((e = dalloc(&d_t, 8 * (size_t)total)) || (e = dalloc(&d_m, 8 * (size_t)total)) ||
+            (e = dalloc(&d_off, 8 * (size_t)(n_lc + 1))) || (e = dalloc(&d_p, 8 * (size_t)n_p)) ||
+            (e = dalloc(&d_pd, 8 * (size_t)n_pdot)) || (e = dalloc(&d_ws, ws_bytes)) ||
+            (e = dalloc(&d_sl[0], slice_bytes)) || (e = dalloc(&d_sl[1], slice_bytes)) ||
+            (e = dalloc(&d_part, 8 * W * (size_t)n_lc * (size_t)n_chunks)) || (e = dalloc(&d_idx, 8 * (size_t)n_lc * k)) ||
+            (e = dalloc(&d_bce, 4 * (size_t)n_lc * k)) || (e = dalloc(&d_st, 32 * (size_t)n_lc))) { rc = cuda_fail(e); break; }
+        cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d_p, periods, 8 * (size_t)n_p, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st);
+        int n_done = 0;
+        for (int c = 0; c < n_chunks && rc == GCE_CE_OK; ++c) {
+            const int64_t a = (int64_t)c * chunk, b = a + chunk < n_p ? a + chunk : n_p;
+            if (a >= b) break;
+            const int buf = c & 1;
+            if (c >= 2) cudaStreamWaitEvent(st, ev_free[buf], 0);  // the copy that last read this slice buffer is done
+            rc = gce_ce_search_partial((const double *)d_t, (const double *)d_m, (const int64_t *)d_off, n_lc, total,
+                                       (const double *)d_p, n_p, (const double *)d_pd, n_pdot, prm, a, b, d_sl[buf],
+                                       (int64_t *)d_part + (size_t)c * (size_t)n_lc * W, d_ws, ws_bytes, st);
+            if (rc) break;
+            ++n_done;
+            cudaEventRecord(ev_done[buf], st);
+            cudaStreamWaitEvent(st2, ev_done[buf], 0);
+            const size_t width = (size_t)(b - a) * (size_t)n_pdot * esz;  // one light curve's rows of this slice
+            e = cudaMemcpy2DAsync(static_cast<unsigned char *>(out_ce) + (size_t)a * (size_t)n_pdot * esz,
+                                  (size_t)n_p * (size_t)n_pdot * esz, d_sl[buf], width, width, (size_t)n_lc,
+                                  cudaMemcpyDeviceToHost, st2);
+            if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+            cudaEventRecord(ev_free[buf], st2);
+        }
+        if (rc) break;
+        if (k || prm->want_stats) {
+            rc = gce_ce_merge_partials((const int64_t *)d_part, n_done, n_lc, prm, out_best_idx ? (int64_t *)d_idx : nullptr,
+                                       out_best_ce ? (float *)d_bce : nullptr, out_stats ? (double *)d_st : nullptr, st);
+            if (rc) break;
+        }
+        if (out_best_idx && k) cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
+        if (out_best_ce && k) cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
+        if (out_stats) cudaMemcpyAsync(out_stats, d_st, 32 * (size_t)n_lc, cudaMemcpyDeviceToHost, st);
+    } while (0);
+    e = cudaStreamSynchronize(st2);
+    if (e != cudaSuccess && rc == GCE_CE_OK) rc = cuda_fail(e);
+    void *frees[] = {d_t, d_m, d_off, d_p, d_pd, d_ws, d_sl[0], d_sl[1], d_part, d_idx, d_bce, d_st};
+    for (void *p : frees)
+        if (p) cudaFreeAsync(p, st);
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess && rc == GCE_CE_OK) rc = cuda_fail(e);
+    for (int b = 0; b < 2; ++b) { cudaEventDestroy(ev_done[b]); cudaEventDestroy(ev_free[b]); }
+    cudaStreamDestroy(st2);
+    cudaStreamDestroy(st);
+    return rc;
+}
+
 int gce_ce_search_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                        const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
                        const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
@@ -1369,6 +1452,14 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
     const int64_t total = lc_offsets[n_lc];
     rc = check_sizes(n_lc, total, n_p, n_pdot);
     if (rc) return rc;
+    if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
+    if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
+    if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+    // a cube of at least 64 MB over at least 64 periods: overlap its transfer with the search, 8 chunks
+    if (out_ce && n_lc > 0 && total > 0 && n_p >= 64 &&
+        (size_t)n_lc * (size_t)n_p * (size_t)n_pdot * (prm->ce_fp64 ? 8 : 4) >= ((size_t)64 << 20))
+        return search_host_pipelined(times, mags, lc_offsets, n_lc, total, periods, n_p, pdots, n_pdot, prm, out_ce,
+                                     out_best_idx, out_best_ce, out_stats, 8);
     size_t ws_bytes = 0;
     rc = gce_ce_workspace_bytes(total, n_lc, n_p, n_pdot, prm, &ws_bytes);
     if (rc) return rc;

@@ -98,3 +98,26 @@ def test_empty_range_and_errors(gce):
     with pytest.raises(gce.GceError) as e:
         gce.gce_ce_search_partial(*args, prm, 40, 51, parts[0], None, ws)
     assert e.value.code == -2
+
+
+def test_host_entry_pipelines_large_cubes_bit_exactly(gce):
+    """gce_ce_search_host with a cube >= 64 MB splits the period axis into chunks and overlaps the device-to-host copy
+    of each slice with the next chunk's search; outputs equal the single device call bit for bit."""
+    w = W.make("C3", n_lc=6, n_p=45001, n_pdot=64)      # 69 MB fp32 cube, ragged last chunk
+    prm = gce.make_params(20, 10, top_k=3, want_stats=True)
+    ce = np.empty((6, 45001, 64), dtype=np.float32)
+    idx = np.empty((6, 3), dtype=np.int64)
+    val = np.empty((6, 3), dtype=np.float32)
+    st = np.empty((6, 4), dtype=np.float64)
+    gce.gce_ce_search_host(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, prm, ce, idx, val, st)
+    res = gce.search(d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), 20, 10, top_k=3, want_cube=True,
+                     want_stats=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(ce, res.ce.cpu().numpy())
+    assert np.array_equal(idx, res.best_idx.cpu().numpy()) and np.array_equal(val, res.best_ce.cpu().numpy())
+    assert np.array_equal(st, res.stats.cpu().numpy())
+    # cube only (no selection, no statistics)
+    prm0 = gce.make_params(20, 10)
+    ce2 = np.zeros_like(ce)
+    gce.gce_ce_search_host(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, prm0, ce2, None, None, None)
+    assert np.array_equal(ce2, ce)
