@@ -1,6 +1,7 @@
 """In-tree build of the C-ABI CUDA library (nvcc, sm_100a only).
 
-`python -m paper_2006_06866_b200.build` or `build()` compiles csrc/gce_ce.cu into
+`python -m paper_2006_06866_b200.build` or `build()` compiles csrc/gce_ce.cu (one translation unit that includes
+csrc/gce_*.cuh) into
 paper_2006_06866_b200/libgce_ce.so.  nvcc cross-compiles without a GPU.  -fmad=false is part of the
 arithmetic contract: a contracted multiply-add would change phase-bin indices.
 """
@@ -28,7 +29,9 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(p) > t for p in (SRC, HDR, os.path.abspath(__file__)))
+    csrc = os.path.dirname(SRC)
+    deps = [os.path.join(csrc, f) for f in os.listdir(csrc) if f.endswith((".cu", ".cuh"))]
+    return any(os.path.getmtime(p) > t for p in (*deps, HDR, os.path.abspath(__file__)))
 
 
 def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:

@@ -1,0 +1,505 @@
+// gce_search.cuh -- S2..S5: the fold + bin + entropy kernel (k_search)
+// Part of the single translation unit gce_ce.cu (compiled with -fmad=false); see the header comment there.
+#pragma once
+#include "gce_common.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------ S2..S5
+__device__ __forceinline__ void red_add_u32(uint32_t addr, uint32_t inc) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(inc) : "memory");
+}
+
+// read-and-clear of one counter word in one LSU instruction (ATOMS.EXCH)
+__device__ __forceinline__ uint32_t exch0_u32(uint32_t addr) {
+    uint32_t w;
+    asm volatile("atom.shared.exch.b32 %0, [%1], %2;" : "=r"(w) : "r"(addr), "r"(0u) : "memory");
+    return w;
+}
+
+// L(k) = k ln k in 2^-42 fixed point for the two 16-bit counter fields of a word.  The fields count in units of
+// 2^us: us = 3 whenever every count of the light curve fits 13 bits (N, or 2N with overlapping bins, <= 8191), so that a
+// field IS the byte offset of its table entry.  BIG = false: the caller guarantees us == 3 and counts < kLtabSmem (a
+// bound on the number of points that can be in the cell): mask / shift, one LDS.64 each.  BIG = true: any us, first
+// kLtabSmem entries from shared memory, the rest from global.
+template <bool BIG>
+__device__ __forceinline__ void ltab_pair(const int64_t *__restrict__ sL, const int64_t *__restrict__ gL, const uint32_t w,
+                                          const uint32_t us, int64_t &v0, int64_t &v1) {
+    if (!BIG) {
+        const unsigned char *b = reinterpret_cast<const unsigned char *>(sL);
+        v0 = *reinterpret_cast<const int64_t *>(b + (w & 0xfff8u));
+        v1 = *reinterpret_cast<const int64_t *>(b + (w >> 16));
+    } else {
+        const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
+        v0 = sL[c0 & (kLtabSmem - 1)];
+        v1 = sL[c1 & (kLtabSmem - 1)];
+        if (c0 >= (uint32_t)kLtabSmem) v0 = gL[c0];
+        if (c1 >= (uint32_t)kLtabSmem) v1 = gL[c1];
+    }
+}
+
+// S2 + S3 for one point and the R trials of this thread (DESIGN.md section 3; PAPER.md:100 Eq. 3, :106).
+//   a = dt*invP ; b = dt2*c ; x = a + b ; y = x*n_phi          (RN each, never fused)
+//   j = floor(y) - n_phi*floor(x)                               two exact round-down magic adds, |y| < 2^51
+// j equals floor(y) mod n_phi except when RN(x*n_phi) lands exactly on the next multiple of n_phi, where it is
+// n_phi: that count goes to an extra histogram row that is folded into row 0 when the segment is closed.
+// PZ: every trial of the thread has c = +-0, so x = a bit for bit (a >= +0) and two operations are skipped.
+template <int R, bool SHARE_P, bool PZ>
+__device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
+                                             const double nphi_d, const uint32_t negn, const uint32_t rs,
+                                             const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0, const uint32_t inc1) {
+    double a;
+    if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
+        const double x = PZ ? a : __dadd_rn(a, __dmul_rn(p.y, cc[r]));
+        const double y = __dmul_rn(x, nphi_d);
+        const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
+        const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
+        const uint32_t j = Iy + Ix * negn;
+        red_add_u32(j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
+    }
+}
+
+// Hot loop over the points [kk, ke) of one shared-memory buffer (all of one magnitude bin).  The next two points are
+// loaded before the current two are folded (the RED asm statements are compiler barriers, so the loads would otherwise
+// sit behind the previous iteration's atomics and the first DMUL would wait for them); the last trip reads up to two
+// entries past ke, which are inside the buffer's slack and never used.
+template <int R, bool SHARE_P, bool PZ>
+__device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
+                                           const double (&cc)[R], const double nphi_d, const uint32_t negn,
+                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0,
+                                           const uint32_t inc1) {
+    if (ke - kk >= 4) {
+        double2 a0 = sp[kk], a1 = sp[kk + 1];
+        do {
+            const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
+            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            a0 = sp[kk + 4];
+            a1 = sp[kk + 5];
+            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            kk += 4;
+        } while (ke - kk >= 4);
+    }
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+}
+
+// Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
+template <int R, bool SHARE_P>
+__device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ sp, int kk, const int ke,
+                                                   const double (&invP)[R], const double (&cc)[R], const int n_phi,
+                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2],
+                                                   const uint32_t inc0, const uint32_t inc1) {
+    for (; kk < ke; ++kk) {
+        const double2 p = sp[kk];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
+            red_add_u32((uint32_t)j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
+        }
+    }
+}
+
+// S4, first half: close magnitude bin `seg_i`.  fetch_word reads and clears this thread's counter word of phase bin j
+// (two 16-bit counts, trials 2*w2 and 2*w2+1); close_word adds it to the phase marginal and accumulates sum L(n_ij).
+__device__ __forceinline__ uint32_t fetch_word(const int j, const int n_phi, const uint32_t rs, const uint32_t hbw) {
+    uint32_t w = exch0_u32(hbw + (uint32_t)j * rs);
+    if (j == 0) w += exch0_u32(hbw + (uint32_t)n_phi * rs);  // phase bin 0 takes over the overflow row
+    return w;
+}
+
+template <int R, bool DUMP, bool BIG>
+__device__ __forceinline__ void close_word(const uint32_t w, const int j, const int w2, const int n_phi, const uint32_t us,
+                                           int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
+                                           const int lc, const int64_t s0, const bool (&valid)[R], const int seg_i) {
+    int64_t v0, v1;
+    ltab_pair<BIG>(sL, prm.ltab, w, us, v0, v1);
+    S2[2 * w2] += v0;
+    if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
+    if (DUMP) {
+        const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
+        if (valid[2 * w2])
+            prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
+        if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
+            prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * prm.n_m + seg_i] = c1;
+    }
+}
+
+// All phase bins of magnitude bin seg_i.  The phase marginal is a register array (REGM, compile-time n_phi) or a second
+// set of counter rows in shared memory updated with one RED per word (no registers, so more threads fit per SM).
+// With a compile-time n_phi the read-and-clear atomics of kCloseGroup phase bins are issued back to back before
+// their results are used, so their latency overlaps.
+// OVL (NEXT item N2): 50 %-overlapping phase bins -- bin k holds the plain cells k-1 and k (cyclic), so
+// the looked-up count is w[k] + w[k-1] (packed 16-bit pairs; needs 2N <= 65535); the folds and the plain marginal are
+// unchanged, the overlap costs one add per word.
+template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL>
+__device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off, const uint32_t us,
+                                              const uint32_t (&hb)[(R + 1) / 2],
+                                              uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
+                                              const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
+                                              const int64_t s0, const bool (&valid)[R], const int seg_i) {
+    constexpr int RW = (R + 1) / 2;
+    uint32_t prev[RW], first[RW];
+    if (NPHI > 0) {
+        constexpr int NP = NPHI > 0 ? NPHI : 1;
+        constexpr int G = NP % kCloseGroup == 0 ? kCloseGroup : 1;
+#pragma unroll
+        for (int j0 = 0; j0 < NP; j0 += G) {
+            uint32_t w[G][RW];
+#pragma unroll
+            for (int jj = 0; jj < G; ++jj)
+#pragma unroll
+                for (int w2 = 0; w2 < RW; ++w2) w[jj][w2] = fetch_word(j0 + jj, n_phi, rs, hb[w2]);
+#pragma unroll
+            for (int jj = 0; jj < G; ++jj)
+#pragma unroll
+                for (int w2 = 0; w2 < RW; ++w2) {
+                    const uint32_t ww = w[jj][w2];
+                    if (REGM) mg[REGM ? j0 + jj : 0][w2] += ww;
+                    else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, ww);
+                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                    else {
+                        if (j0 + jj == 0) first[w2] = ww;
+                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                        prev[w2] = ww;
+                    }
+                }
+        }
+    } else {
+        for (int j = 0; j < n_phi; ++j) {
+#pragma unroll
+            for (int w2 = 0; w2 < RW; ++w2) {
+                const uint32_t ww = fetch_word(j, n_phi, rs, hb[w2]);
+                red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, ww);
+                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                else {
+                    if (j == 0) first[w2] = ww;
+                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                    prev[w2] = ww;
+                }
+            }
+        }
+    }
+    if (OVL) {  // bin 0 = cells n_phi-1 and 0
+#pragma unroll
+        for (int w2 = 0; w2 < RW; ++w2)
+            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+    }
+}
+
+// NPHI > 0: compile-time n_phi (unrolled S4); NPHI == 0: any n_phi <= 64.  REGM: phase marginal in registers, exactly
+// 512 threads per CTA; otherwise the marginal is a second set of counter rows in shared memory, threads per CTA =
+// prm.nt (any multiple of 32 up to 640), which leaves registers for a fifth warp per sub-partition when the shared
+// memory allows it.  R = trials per thread.  SHARE_P: the R trials of a thread share one period (n_pdot % R == 0).
+// DUMP: test mode, trials come from a list and the count tables are written out.
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP>
+__global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchParams prm) {
+    static_assert(!REGM || NPHI > 0, "register marginals need a compile-time n_phi");
+    constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
+    constexpr int NPHI_REG = REGM ? NPHI : 1;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int NT = REGM ? 512 : (int)blockDim.x, NW = NT >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int n_phi = NPHI > 0 ? NPHI : prm.n_phi, n_m = prm.n_m;
+    const uint32_t rs = (uint32_t)NT * 4u;  // bytes between the counter rows of consecutive phase bins
+
+    // shared-memory carve-up (dynamic part; the L table is static so that lookups are LDS.64 [offset + const]), points last
+    __shared__ __align__(16) int64_t sL[kLtabSmem];  // static: its shared address is a link-time constant
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);                     // [2]
+    int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
+    uint64_t *sstat = reinterpret_cast<uint64_t *>(sseg + GCE_CE_MAX_BINS + 4);  // [kMaxWarps][kStatWords]
+    uint32_t *hist = reinterpret_cast<uint32_t *>(sstat + kMaxWarps * kStatWords); // [RW][n_phi + 1][NT], 16-byte aligned
+    const uint32_t plane = (uint32_t)(n_phi + 1) * rs;                           // bytes per counter-word plane
+    // shared-memory marginal (!REGM): RW planes of n_phi rows after the histogram; word (w2, j) of this thread is at
+    // hb[w2] + marg_off + (j - w2) * rs
+    const uint32_t marg_off = (uint32_t)RW * plane;
+    const uint32_t hist_words = (uint32_t)(REGM ? RW * (n_phi + 1) : RW * (2 * n_phi + 1)) * (uint32_t)NT;
+    double2 *spts = reinterpret_cast<double2 *>(hist + hist_words);              // [cap_points + 2]
+
+    const int lc = blockIdx.x / prm.jobs_per_lc;
+    const int job = blockIdx.x % prm.jobs_per_lc;
+    const int64_t tile_lo = prm.tiles_per_lc * job / prm.jobs_per_lc;
+    const int64_t tile_hi = prm.tiles_per_lc * (job + 1) / prm.jobs_per_lc;
+    const int n_tiles = (int)(tile_hi - tile_lo);
+    const int N = prm.info[lc].n;
+    const double dt_max = prm.info[lc].dt_max;
+    const int64_t K = prm.info[lc].K;
+    const double2 *gpts = prm.pts + prm.lc_offsets[lc];
+    const bool single = N <= prm.cap_points;            // the whole light curve stays resident for every tile
+    const int CH = single ? N : prm.cap_points / 2;     // else: streamed through two half buffers, per tile
+    const int n_chunks = N > 0 ? (N + CH - 1) / CH : 0;
+    const int total_seq = single ? n_chunks : n_tiles * n_chunks;
+    const int64_t TILE = (int64_t)NT * R;
+
+    auto issue_chunk = [&](int g) {  // thread 0 only: TMA bulk copy of sequence element g into its buffer
+        const int c = g % n_chunks, buf = single ? 0 : (g & 1);
+        const int cnt = min(CH, N - c * CH);
+        mbar_expect_tx(&full[buf], (uint32_t)cnt * 16u);
+        for (int o = 0; o < cnt; o += 2048)
+            tma_load_bulk(spts + (size_t)buf * CH + o, gpts + (size_t)c * CH + o, (uint32_t)min(2048, cnt - o) * 16u, &full[buf]);
+    };
+
+    // ---- prologue: zero histograms, stage table / segments, start the point loads
+    for (uint32_t i = tid; i < hist_words; i += NT) hist[i] = 0u;
+    for (int i = tid; i < kLtabSmem; i += NT) sL[i] = i < prm.ltab_n ? prm.ltab[i] : 0;
+    for (int i = tid; i <= n_m; i += NT) sseg[i] = prm.seg[(int64_t)lc * (n_m + 1) + i];
+    if (tid < NW) stat_init(sstat + tid * kStatWords);
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if (n_tiles > 0)
+            for (int g = 0; g < 2 && g < total_seq; ++g) issue_chunk(g);
+    }
+    __syncthreads();
+
+    WarpTopK top;
+    top.reset(prm.top_k > 0 ? prm.top_k : 1);
+
+    const double nphi_d = (double)n_phi;
+    const uint32_t negn = 0u - (uint32_t)n_phi;
+    uint32_t hb[RW];
+#pragma unroll
+    for (int w2 = 0; w2 < RW; ++w2) hb[w2] = smem_u32(hist) + (uint32_t)tid * 4u + (uint32_t)w2 * plane;
+    const bool ovl = !DUMP && prm.overlap != 0;  // N2: 2N table entries per trial
+    const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)(ovl ? 2 * N : N) : 0.0;
+    const uint32_t us = ((ovl ? 2 : 1) * N <= 8191) ? 3u : 0u;  // counter unit 2^us: a field is its table entry's byte offset
+    const uint32_t inc0 = 1u << us, inc1 = 0x10000u << us;
+    uint32_t mg[NPHI_REG][RW];  // phase marginal n_j of the R trials (NPHI > 0), packed like the histogram
+#pragma unroll
+    for (int j = 0; j < NPHI_REG; ++j)
+#pragma unroll
+        for (int w2 = 0; w2 < RW; ++w2) mg[j][w2] = 0u;
+
+    // Warps that share an SM sub-partition (warp id mod 4) start at different magnitude bins, a quarter of the points
+    // apart, so that one warp's S4 (no FP64) overlaps the others' folds (FP64-bound).  Counts and the integer entropy
+    // sums do not depend on the order of the bins.  Streamed light curves are processed in storage order.
+    int rot = 0;
+    if (single && n_m > 1) {
+        const int groups = (NW + 3) >> 2;
+        const int target = (int)((int64_t)N * (tid >> 7) / groups);
+        while (rot + 1 < n_m && sseg[rot + 1] <= target) ++rot;
+    }
+    int g = 0;  // position in this CTA's chunk sequence (streamed mode)
+    for (int tl = 0; tl < n_tiles; ++tl) {
+        const int64_t s0 = (tile_lo + tl) * TILE + (int64_t)tid * R;  // first trial slot of this thread
+        // ---- per-trial constants
+        double invP[R], cc[R];  // SHARE_P: only invP[0] is used
+        int64_t qv[R];
+        bool valid[R];
+        bool fast = true, pz = true;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t s = s0 + r;
+            valid[r] = s < prm.n_trials;
+            int64_t q = 0;
+            if (valid[r]) q = DUMP ? prm.trial_q[s] : s;
+            qv[r] = q + prm.q_off;  // reported index: flat q of the caller's whole grid
+            double ip = 0.0, c = 0.0;
+            if (valid[r] && (!SHARE_P || r == 0)) ip = __ddiv_rn(1.0, prm.periods[q / prm.n_pdot]);
+            if (SHARE_P && r > 0) ip = invP[0];
+            if (valid[r]) c = __dmul_rn(__dmul_rn(__dmul_rn(-0.5, prm.pdots[q % prm.n_pdot]), ip), ip);
+            invP[r] = ip;
+            cc[r] = c;
+            // conservative bound on |y|: below 2^51 the magic-add floors are exact
+            fast = fast && (nphi_d * (dt_max * fabs(ip) + dt_max * dt_max * fabs(c)) * 1.000001 < kYSafe);
+            pz = pz && (c == 0.0);
+        }
+        fast = __all_sync(0xffffffffu, fast);
+        pz = __all_sync(0xffffffffu, pz);
+
+        int64_t S2[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) S2[r] = 0;
+
+        int seg_s = 0;  // magnitude bins finished so far, counted in this warp's (rotated) order
+        for (int c = 0; c < n_chunks; ++c) {
+            const int buf = single ? 0 : (g & 1);
+            if (!single || tl == 0) mbar_wait(&full[buf], single ? 0u : (uint32_t)((g >> 1) & 1));
+            const double2 *sp = spts + (size_t)buf * CH;
+            const int k_base = c * CH;
+            const int k_end = min(N, k_base + CH);
+            while (seg_s < n_m) {
+                int seg_i = seg_s + rot;
+                if (seg_i >= n_m) seg_i -= n_m;
+                const int b0 = sseg[seg_i], b1 = sseg[seg_i + 1];
+                const int lo = max(b0, k_base) - k_base, hi = min(b1, k_end) - k_base;
+                // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
+                if (lo < hi) {
+                    if (fast) {
+                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                    } else {
+                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, inc0, inc1);
+                    }
+                }
+                if (b1 > k_end) break;  // the bin continues in the next buffer
+                // ---------------- S4: the bin is complete; a cell holds at most b1 - b0 points
+                if (b1 > b0) {
+                    // a cell of this bin holds at most b1 - b0 points (twice that with overlapping bins)
+                    if (!ovl) {
+                        if (us == 3u && b1 - b0 < kLtabSmem)
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        else
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                    } else if (!DUMP) {
+                        if (us == 3u && 2 * (b1 - b0) < kLtabSmem)
+                            close_mag_bin<NPHI, REGM, R, false, false, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                        else
+                            close_mag_bin<NPHI, REGM, R, false, true, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                    }
+                }
+                ++seg_s;
+            }
+            if (!single) {  // streamed mode: everyone is done with this half buffer -> refill it with element g + 2
+                __syncthreads();
+                if (tid == 0 && g + 2 < total_seq) issue_chunk(g + 2);
+                ++g;
+            }
+        }
+
+        // ---------------- finish the trials: S1 = sum_j L(n_j), CE, outputs
+        int64_t S1[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) S1[r] = 0;
+        if (N > 0) {
+            auto add_marg = [&](const uint32_t w, const int w2, auto big) {
+                int64_t v0, v1;
+                ltab_pair<decltype(big)::value>(sL, prm.ltab, w, us, v0, v1);
+                S1[2 * w2] += v0;
+                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
+            };
+            auto marg_pass = [&](auto big, auto ovlt) {
+                constexpr bool OVL = decltype(ovlt)::value;
+                uint32_t prev[RW], first[RW];
+                if (REGM) {
+#pragma unroll
+                    for (int j = 0; j < NPHI_REG; ++j)
+#pragma unroll
+                        for (int w2 = 0; w2 < RW; ++w2) {
+                            const uint32_t ww = mg[j][w2];
+                            mg[j][w2] = 0u;
+                            if (!OVL) add_marg(ww, w2, big);
+                            else { if (j == 0) first[w2] = ww; else add_marg(ww + prev[w2], w2, big); prev[w2] = ww; }
+                        }
+                } else {
+                    for (int j = 0; j < n_phi; ++j)
+#pragma unroll
+                        for (int w2 = 0; w2 < RW; ++w2) {
+                            const uint32_t ww = exch0_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs);
+                            if (!OVL) add_marg(ww, w2, big);
+                            else { if (j == 0) first[w2] = ww; else add_marg(ww + prev[w2], w2, big); prev[w2] = ww; }
+                        }
+                }
+                if (OVL) {
+#pragma unroll
+                    for (int w2 = 0; w2 < RW; ++w2) add_marg(first[w2] + prev[w2], w2, big);
+                }
+            };
+            if (!ovl) { if (us == 3u && N < kLtabSmem) marg_pass(FalseT{}, FalseT{}); else marg_pass(TrueT{}, FalseT{}); }
+            else { if (us == 3u && 2 * N < kLtabSmem) marg_pass(FalseT{}, TrueT{}); else marg_pass(TrueT{}, TrueT{}); }
+        }
+        double ce[R];
+        int64_t S[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            S[r] = S1[r] - S2[r];  // = N * CE * 2^42, exact
+            ce[r] = N > 0 ? (double)S[r] * ce_scale : CUDART_NAN;
+        }
+        if (DUMP) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (valid[r] && prm.out_ce_at) prm.out_ce_at[(int64_t)lc * prm.n_trials + s0 + r] = ce[r];
+        } else {
+            if (prm.out_ce) {
+                const int64_t o = (int64_t)lc * prm.n_trials + s0;  // q == slot outside DUMP
+                float *o32 = reinterpret_cast<float *>(prm.out_ce) + o;
+                if (R == 4 && !prm.ce_fp64 && valid[R - 1] && (reinterpret_cast<uintptr_t>(o32) & 15u) == 0) {
+                    *reinterpret_cast<float4 *>(o32) = make_float4((float)ce[0], (float)ce[1 % R], (float)ce[2 % R], (float)ce[3 % R]);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        if (!valid[r]) continue;
+                        if (prm.ce_fp64) reinterpret_cast<double *>(prm.out_ce)[o + r] = ce[r];
+                        else o32[r] = (float)ce[r];
+                    }
+                }
+            }
+            if (prm.top_k > 0) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) top.offer((valid[r] && N > 0) ? S[r] : kInfS, (valid[r] && N > 0) ? qv[r] : kInfS);
+            }
+            if (prm.part_stats != nullptr && N > 0) {  // Eq. 5 partial sums of this tile, warp-reduced, exact integers
+                __int128 a = 0;
+                u128_t b = 0;
+                int64_t mn = kInfS, mx = INT64_MIN;
+                uint32_t cnt = 0;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (!valid[r]) continue;
+                    const int64_t d = S[r] - K;   // |d| < 2^60
+                    a += d;
+                    b += (u128_t)((__int128)d * d);
+                    mn = S[r] < mn ? S[r] : mn;
+                    mx = S[r] > mx ? S[r] : mx;
+                    ++cnt;
+                }
+                u128_t au = (u128_t)a;
+                for (int o = 16; o > 0; o >>= 1) {
+                    au += shfl_xor_u128(au, o);
+                    b += shfl_xor_u128(b, o);            // <= 32 * R * 2^120 < 2^128
+                    const int64_t m2 = __shfl_xor_sync(0xffffffffu, mn, o), m3 = __shfl_xor_sync(0xffffffffu, mx, o);
+                    mn = m2 < mn ? m2 : mn;
+                    mx = m3 > mx ? m3 : mx;
+                    cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+                }
+                if (lane == 0) stat_add(sstat + (tid >> 5) * kStatWords, cnt, au, b, 0, mn, mx);
+            }
+        }
+    }
+
+    // ---------------- per-CTA Eq. 5 partial sums -> part_stats[lc][job]
+    if (!DUMP && prm.part_stats != nullptr) {
+        __syncthreads();
+        if (tid == 0) {
+            uint64_t tot[kStatWords];
+            stat_init(tot);
+            for (int w = 0; w < NW; ++w) stat_merge(tot, sstat + w * kStatWords);
+            uint64_t *o = prm.part_stats + ((int64_t)lc * prm.jobs_per_lc + job) * kStatWords;
+            for (int i = 0; i < kStatWords; ++i) o[i] = tot[i];
+        }
+    }
+
+    // ---------------- per-CTA merge of the warps' top-k lists -> partial[lc][job][k]
+    if (!DUMP && prm.top_k > 0) {
+        const int K = prm.top_k;
+        __syncthreads();  // every issued TMA load has been consumed: the point buffer is idle, reuse it as scratch
+        int64_t *scr = reinterpret_cast<int64_t *>(spts);  // 16 * NW * K <= 10 KB <= cap_points * 16 (cap >= kMinPoints)
+        if (lane < K) {
+            scr[2 * ((tid >> 5) * K + lane)] = top.S;
+            scr[2 * ((tid >> 5) * K + lane) + 1] = top.q;
+        }
+        __syncthreads();
+        if (tid < 32) {
+            top.reset(K);
+            for (int e = 0; e < NW * K; e += 32) {
+                const int i = e + lane;
+                const int64_t cS = i < NW * K ? scr[2 * i] : kInfS;
+                const int64_t cq = i < NW * K ? scr[2 * i + 1] : kInfS;
+                top.offer(cS, cq);
+            }
+            if (lane < K) {
+                const int64_t o = ((int64_t)lc * prm.jobs_per_lc + job) * K + lane;
+                prm.part_S[o] = top.S;
+                prm.part_q[o] = top.q;
+            }
+        }
+    }
+}
+
+
+}  // namespace
