@@ -45,9 +45,10 @@ FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (DESIG
 N_SM = 148
 OVERLAP = [False]   # set from --overlap; the oracle legs time the same binning
 # DRAM traffic of one k_search launch from the committed ncu --set full capture (profiles/r1_k_search_C3_full.md):
-# 17.1 MB read + 773.2 MB written; the algorithmic output is the 819.2 MB fp32 cube (part of it is still in L2 at
-# kernel end).  Only workloads that were captured have an entry.
-NCU_DRAM_BYTES_PER_LAUNCH = {"C3": 17.1e6 + 773.2e6}
+# C3: 15.9 MB read + 774.0 MB written (the algorithmic output is the 819.2 MB fp32 cube; part of it is still in L2 at
+# kernel end); C5 (profiles/r1_k_search_C5_full.md, no cube): 2.5 MB read, 256 B written.  Only workloads that were
+# captured have an entry.
+NCU_DRAM_BYTES_PER_LAUNCH = {"C3": 15.9e6 + 774.0e6, "C5": 2.5e6}
 
 
 def load_peaks():
@@ -318,7 +319,7 @@ def run_ours(args):
             "unit": "G FP64 lane-ops/s", "frac": achieved / peak,
             "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if not args.quick else None,
             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_search launch, ncu --set full "
-                              "(profiles/r1_k_search_C3_full.md); bytes per launch",
+                              "(profiles/r1_k_search_C3_full.md, r1_k_search_C5_full.md); bytes per launch",
             "peak_source": f"64 FP64 lanes/SM/clk x 148 SMs x {sm_max:.0f} MHz (max SM clock, {peaks_src} MEASURED_PEAKS.json; "
                            "per-SM rate probe-measured, DESIGN.md section 7)",
             "algorithmic_ops_per_point_fold": algorithmic_fp64_ops_per_pointfold(w),
