@@ -44,12 +44,35 @@ __device__ __forceinline__ void ltab_pair(const int64_t *__restrict__ sL, const 
 // j equals floor(y) mod n_phi except when RN(x*n_phi) lands exactly on the next multiple of n_phi, where it is
 // n_phi: that count goes to an extra histogram row that is folded into row 0 when the segment is closed.
 // PZ: every trial of the thread has c = +-0, so x = a bit for bit (a >= +0) and two operations are skipped.
-template <int R, bool SHARE_P, bool PZ>
+// PAIR (only with extended counter rows, EXT in k_search): the two trials of a counter word share one floor(x).  The
+// caller has ordered each pair so that the odd slot has the smaller c and has checked (c_even - c_odd) * dt_max^2 < 1,
+// hence x_odd <= x_even < x_odd + 1 for every point and both j = floor(y) - n_phi * floor(x_odd) lie in [0, 2 n_phi]:
+// rows n_phi .. 2 n_phi are folded back (mod n_phi) when the magnitude bin is closed.  One FP64 instruction fewer per
+// two point-folds, the same bits.
+template <int R, bool SHARE_P, bool PZ, bool PAIR>
 __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
                                              const double nphi_d, const uint32_t negn, const uint32_t rs,
                                              const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0, const uint32_t inc1) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
+    if (PAIR) {
+        static_assert(!PAIR || (SHARE_P && !PZ && R % 2 == 0), "pairs share a period and have Pdot != 0");
+        double x[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) x[r] = __dadd_rn(a, __dmul_rn(p.y, cc[r]));
+#pragma unroll
+        for (int r = 0; r < R; r += 2) {
+            const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x[(r + 1) % R], kMagic));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const double y = __dmul_rn(x[(r + h) % R], nphi_d);
+                const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
+                const uint32_t j = Iy + Ix * negn;
+                red_add_u32(j * rs + hb[r >> 1], h ? inc1 : inc0);
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
@@ -62,11 +85,7 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
     }
 }
 
-// Hot loop over the points [kk, ke) of one shared-memory buffer (all of one magnitude bin).  The next two points are
-// loaded before the current two are folded (the RED asm statements are compiler barriers, so the loads would otherwise
-// sit behind the previous iteration's atomics and the first DMUL would wait for them); the last trip reads up to two
-// entries past ke, which are inside the buffer's slack and never used.
-template <int R, bool SHARE_P, bool PZ>
+template <int R, bool SHARE_P, bool PZ, bool PAIR>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
                                            const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0,
@@ -75,16 +94,16 @@ __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int k
         double2 a0 = sp[kk], a1 = sp[kk + 1];
         do {
             const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-            fold_bin_add<R, SHARE_P, PZ>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-            fold_bin_add<R, SHARE_P, PZ>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, PAIR>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, PAIR>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
             a0 = sp[kk + 4];
             a1 = sp[kk + 5];
-            fold_bin_add<R, SHARE_P, PZ>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-            fold_bin_add<R, SHARE_P, PZ>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, PAIR>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, PAIR>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
             kk += 4;
         } while (ke - kk >= 4);
     }
-    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, PAIR>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
 }
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
@@ -105,9 +124,11 @@ __device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ s
 
 // S4, first half: close magnitude bin `seg_i`.  fetch_word reads and clears this thread's counter word of phase bin j
 // (two 16-bit counts, trials 2*w2 and 2*w2+1); close_word adds it to the phase marginal and accumulates sum L(n_ij).
+template <bool EXT>
 __device__ __forceinline__ uint32_t fetch_word(const int j, const int n_phi, const uint32_t rs, const uint32_t hbw) {
     uint32_t w = exch0_u32(hbw + (uint32_t)j * rs);
-    if (j == 0) w += exch0_u32(hbw + (uint32_t)n_phi * rs);  // phase bin 0 takes over the overflow row
+    if (EXT) w += exch0_u32(hbw + (uint32_t)(j + n_phi) * rs);  // extended rows n_phi .. 2 n_phi - 1 fold back mod n_phi
+    if (j == 0) w += exch0_u32(hbw + (uint32_t)(EXT ? 2 * n_phi : n_phi) * rs);  // phase bin 0 takes over the last row
     return w;
 }
 
@@ -135,7 +156,7 @@ __device__ __forceinline__ void close_word(const uint32_t w, const int j, const 
 // OVL (NEXT item N2): 50 %-overlapping phase bins -- bin k holds the plain cells k-1 and k (cyclic), so
 // the looked-up count is w[k] + w[k-1] (packed 16-bit pairs; needs 2N <= 65535); the folds and the plain marginal are
 // unchanged, the overlap costs one add per word.
-template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL>
+template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL, bool EXT>
 __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off, const uint32_t us,
                                               const uint32_t (&hb)[(R + 1) / 2],
                                               uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
@@ -152,7 +173,7 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
 #pragma unroll
             for (int jj = 0; jj < G; ++jj)
 #pragma unroll
-                for (int w2 = 0; w2 < RW; ++w2) w[jj][w2] = fetch_word(j0 + jj, n_phi, rs, hb[w2]);
+                for (int w2 = 0; w2 < RW; ++w2) w[jj][w2] = fetch_word<EXT>(j0 + jj, n_phi, rs, hb[w2]);
 #pragma unroll
             for (int jj = 0; jj < G; ++jj)
 #pragma unroll
@@ -172,7 +193,7 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
         for (int j = 0; j < n_phi; ++j) {
 #pragma unroll
             for (int w2 = 0; w2 < RW; ++w2) {
-                const uint32_t ww = fetch_word(j, n_phi, rs, hb[w2]);
+                const uint32_t ww = fetch_word<EXT>(j, n_phi, rs, hb[w2]);
                 red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, ww);
                 if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
                 else {
@@ -195,9 +216,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
 // prm.nt (any multiple of 32 up to 640), which leaves registers for a fifth warp per sub-partition when the shared
 // memory allows it.  R = trials per thread.  SHARE_P: the R trials of a thread share one period (n_pdot % R == 0).
 // DUMP: test mode, trials come from a list and the count tables are written out.
-template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP>
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT>
 __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchParams prm) {
     static_assert(!REGM || NPHI > 0, "register marginals need a compile-time n_phi");
+    static_assert(!EXT || (SHARE_P && !DUMP && R % 2 == 0), "extended rows serve trial pairs that share a period");
     constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
     constexpr int NPHI_REG = REGM ? NPHI : 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -212,11 +234,12 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
     uint64_t *sstat = reinterpret_cast<uint64_t *>(sseg + GCE_CE_MAX_BINS + 4);  // [kMaxWarps][kStatWords]
     uint32_t *hist = reinterpret_cast<uint32_t *>(sstat + kMaxWarps * kStatWords); // [RW][n_phi + 1][NT], 16-byte aligned
-    const uint32_t plane = (uint32_t)(n_phi + 1) * rs;                           // bytes per counter-word plane
+    const int hist_rows = EXT ? 2 * n_phi + 1 : n_phi + 1;  // EXT: a pair's shared floor(x) lets j reach 2 n_phi
+    const uint32_t plane = (uint32_t)hist_rows * rs;                             // bytes per counter-word plane
     // shared-memory marginal (!REGM): RW planes of n_phi rows after the histogram; word (w2, j) of this thread is at
     // hb[w2] + marg_off + (j - w2) * rs
     const uint32_t marg_off = (uint32_t)RW * plane;
-    const uint32_t hist_words = (uint32_t)(REGM ? RW * (n_phi + 1) : RW * (2 * n_phi + 1)) * (uint32_t)NT;
+    const uint32_t hist_words = (uint32_t)(REGM ? RW * hist_rows : RW * (hist_rows + n_phi)) * (uint32_t)NT;
     double2 *spts = reinterpret_cast<double2 *>(hist + hist_words);              // [cap_points + 2]
 
     const int lc = blockIdx.x / prm.jobs_per_lc;
@@ -311,6 +334,24 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
         }
         fast = __all_sync(0xffffffffu, fast);
         pz = __all_sync(0xffffffffu, pz);
+        // EXT: order each pair so that the odd slot has the smaller c (= the smaller x for every point, dt2 >= 0) and
+        // check that the pair's phases stay less than one cycle apart over the whole light curve
+        bool swp[RW];
+        bool pair_ok = EXT && fast && !pz;
+        if (EXT) {
+#pragma unroll
+            for (int w2 = 0; w2 < RW; ++w2) {
+                const int e = 2 * w2, o = (2 * w2 + 1) % R;
+                swp[w2] = cc[e] < cc[o];
+                if (swp[w2]) {
+                    const double tc = cc[e]; cc[e] = cc[o]; cc[o] = tc;
+                    const int64_t tq = qv[e]; qv[e] = qv[o]; qv[o] = tq;
+                    const bool tv = valid[e]; valid[e] = valid[o]; valid[o] = tv;
+                }
+                pair_ok = pair_ok && ((cc[e] - cc[o]) * dt_max * dt_max < 0.999);
+            }
+            pair_ok = __all_sync(0xffffffffu, pair_ok);
+        }
 
         int64_t S2[R];
 #pragma unroll
@@ -331,8 +372,9 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-                        if (pz) fold_range<R, SHARE_P, true>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-                        else fold_range<R, SHARE_P, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        if (pz) fold_range<R, SHARE_P, true, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else fold_range<R, SHARE_P, false, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
                     } else {
                         fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, inc0, inc1);
                     }
@@ -343,14 +385,14 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                     // a cell of this bin holds at most b1 - b0 points (twice that with overlapping bins)
                     if (!ovl) {
                         if (us == 3u && b1 - b0 < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, DUMP, false, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, DUMP, true, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                     } else if (!DUMP) {
                         if (us == 3u && 2 * (b1 - b0) < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, false, false, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, false, false, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, false, true, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, false, true, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
                     }
                 }
                 ++seg_s;
@@ -418,14 +460,17 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
             if (prm.out_ce) {
                 const int64_t o = (int64_t)lc * prm.n_trials + s0;  // q == slot outside DUMP
                 float *o32 = reinterpret_cast<float *>(prm.out_ce) + o;
-                if (R == 4 && !prm.ce_fp64 && valid[R - 1] && (reinterpret_cast<uintptr_t>(o32) & 15u) == 0) {
-                    *reinterpret_cast<float4 *>(o32) = make_float4((float)ce[0], (float)ce[1 % R], (float)ce[2 % R], (float)ce[3 % R]);
+                double cet[R];  // CE in trial order (EXT may have swapped the slots of a pair)
+#pragma unroll
+                for (int r = 0; r < R; ++r) cet[r] = (EXT && swp[r >> 1]) ? ce[(r ^ 1) % R] : ce[r];
+                if (R == 4 && !prm.ce_fp64 && s0 + R <= prm.n_trials && (reinterpret_cast<uintptr_t>(o32) & 15u) == 0) {
+                    *reinterpret_cast<float4 *>(o32) = make_float4((float)cet[0], (float)cet[1 % R], (float)cet[2 % R], (float)cet[3 % R]);
                 } else {
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        if (!valid[r]) continue;
-                        if (prm.ce_fp64) reinterpret_cast<double *>(prm.out_ce)[o + r] = ce[r];
-                        else o32[r] = (float)ce[r];
+                        if (s0 + r >= prm.n_trials) continue;
+                        if (prm.ce_fp64) reinterpret_cast<double *>(prm.out_ce)[o + r] = cet[r];
+                        else o32[r] = (float)cet[r];
                     }
                 }
             }

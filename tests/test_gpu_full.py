@@ -317,3 +317,33 @@ def test_overlap_paper_binning_sampled_at_c3_size(gce, oracle):
         assert set(q[better].tolist()) <= set(idx[lc].tolist())
     st = res.stats.cpu().numpy()
     assert np.allclose(st[:, 2], val[:, 0].astype(np.float64), rtol=1e-6) and np.all(st[:, 1] > 0)
+
+
+# ------------------------------------------------------------------------------------------ extended-row variant (pair floors)
+@pytest.mark.parametrize("n_phi,pdots", [
+    (20, np.linspace(-1e-10, 0.0, 64)),                       # C3's own grid: every pair within one cycle
+    (20, np.linspace(0.0, -1e-10, 64)),                       # descending Pdot: the other slot of each pair is the base
+    (20, np.linspace(-5e-9, 5e-9, 8)),                        # both signs, pairs more than a cycle apart at short periods:
+                                                              # the warp falls back to its own floor per trial there
+    (15, np.random.default_rng(5).permutation(np.linspace(-3e-10, 1e-10, 16))),   # unordered Pdots: mixed swaps
+    (20, np.array([-1e-10, -1e-10, -1e-10, 0.0])),            # equal Pdots inside a pair, Pdot = 0 inside a thread
+])
+def test_pair_floor_variant_matches_oracle(gce, oracle, n_phi, pdots):
+    """k_search's extended-row variant (two trials of a counter word share one floor(x), rows up to 2 n_phi folded back
+    when the bin closes) against the oracle: fp64 cube to 1e-12, top-k, Eq. 5; odd tile tails and a short light curve."""
+    w = W.make("C3", n_lc=3, n_p=1531, n_pdot=4)
+    pd = np.ascontiguousarray(pdots, dtype=np.float64)
+    n_m = 10 if n_phi == 20 else 8
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, pd, n_phi, n_m)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(pd), n_phi, n_m, top_k=4, want_cube=True,
+                     ce_fp64=True, want_stats=True)
+    torch.cuda.synchronize()
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    for lc in range(w.n_lc):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 4, RTOL64, oracle)
+    np.testing.assert_allclose(res.stats.cpu().numpy(), _stats_ref(oracle, ref.reshape(w.n_lc, -1)), rtol=RTOL_STATS)
+    res32 = gce.search(d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(pd), n_phi, n_m, top_k=4, want_cube=True)
+    torch.cuda.synchronize()
+    assert_ce_close(res32.ce.cpu().numpy(), ref, RTOL32)
+    assert torch.equal(res32.best_idx, res.best_idx)
