@@ -44,31 +44,36 @@ __device__ __forceinline__ void ltab_pair(const int64_t *__restrict__ sL, const 
 // j equals floor(y) mod n_phi except when RN(x*n_phi) lands exactly on the next multiple of n_phi, where it is
 // n_phi: that count goes to an extra histogram row that is folded into row 0 when the segment is closed.
 // PZ: every trial of the thread has c = +-0, so x = a bit for bit (a >= +0) and two operations are skipped.
-// PAIR (only with extended counter rows, EXT in k_search): the two trials of a counter word share one floor(x).  The
-// caller has ordered each pair so that the odd slot has the smaller c and has checked (c_even - c_odd) * dt_max^2 < 1,
-// hence x_odd <= x_even < x_odd + 1 for every point and both j = floor(y) - n_phi * floor(x_odd) lie in [0, 2 n_phi]:
-// rows n_phi .. 2 n_phi are folded back (mod n_phi) when the magnitude bin is closed.  One FP64 instruction fewer per
-// two point-folds, the same bits.
-template <int R, bool SHARE_P, bool PZ, bool PAIR>
+// MODE 1 / 2 (only with extended counter rows, EXT in k_search): trials share a floor(x).  The caller has sorted the
+// thread's trials by c, largest first, so that for every point x_0 >= x_1 >= ... (dt2 >= 0, RN is monotone), and has
+// checked per tile that the trials sharing a floor stay less than one cycle apart over the whole light curve:
+//   MODE 1: the two trials of a counter word share floor(x) of the odd slot   ((c_even - c_odd) * dt_max^2 < 1)
+//   MODE 2: all R trials share floor(x) of the last slot                       ((c_0 - c_{R-1}) * dt_max^2 < 1)
+// Then every j = floor(y) - n_phi * floor(x_base) lies in [0, 2 n_phi]; rows n_phi .. 2 n_phi are folded back (mod
+// n_phi) when the magnitude bin is closed.  Fewer FP64 instructions and one row-offset multiply-add per counter word
+// instead of per trial, the same bits.
+template <int R, bool SHARE_P, bool PZ, int MODE>
 __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
                                              const double nphi_d, const uint32_t negn, const uint32_t rs,
                                              const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0, const uint32_t inc1) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
-    if (PAIR) {
-        static_assert(!PAIR || (SHARE_P && !PZ && R % 2 == 0), "pairs share a period and have Pdot != 0");
+    if (MODE != 0) {
+        static_assert(MODE == 0 || (SHARE_P && !PZ && R % 2 == 0), "shared floors need one period and Pdot != 0");
         double x[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = __dadd_rn(a, __dmul_rn(p.y, cc[r]));
+        uint32_t Ix = 0;
+        if (MODE == 2) Ix = (uint32_t)__double2loint(__dadd_rd(x[R - 1], kMagic));
 #pragma unroll
         for (int r = 0; r < R; r += 2) {
-            const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x[(r + 1) % R], kMagic));
+            if (MODE == 1) Ix = (uint32_t)__double2loint(__dadd_rd(x[(r + 1) % R], kMagic));
+            const uint32_t base = Ix * (negn * rs) + hb[r >> 1];  // one multiply-add for the word's common row offset
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const double y = __dmul_rn(x[(r + h) % R], nphi_d);
                 const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
-                const uint32_t j = Iy + Ix * negn;
-                red_add_u32(j * rs + hb[r >> 1], h ? inc1 : inc0);
+                red_add_u32(Iy * rs + base, h ? inc1 : inc0);
             }
         }
         return;
@@ -85,7 +90,7 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
     }
 }
 
-template <int R, bool SHARE_P, bool PZ, bool PAIR>
+template <int R, bool SHARE_P, bool PZ, int MODE>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
                                            const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0,
@@ -94,16 +99,16 @@ __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int k
         double2 a0 = sp[kk], a1 = sp[kk + 1];
         do {
             const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-            fold_bin_add<R, SHARE_P, PZ, PAIR>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-            fold_bin_add<R, SHARE_P, PZ, PAIR>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
             a0 = sp[kk + 4];
             a1 = sp[kk + 5];
-            fold_bin_add<R, SHARE_P, PZ, PAIR>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-            fold_bin_add<R, SHARE_P, PZ, PAIR>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
             kk += 4;
         } while (ke - kk >= 4);
     }
-    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, PAIR>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
 }
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
@@ -334,23 +339,29 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
         }
         fast = __all_sync(0xffffffffu, fast);
         pz = __all_sync(0xffffffffu, pz);
-        // EXT: order each pair so that the odd slot has the smaller c (= the smaller x for every point, dt2 >= 0) and
-        // check that the pair's phases stay less than one cycle apart over the whole light curve
-        bool swp[RW];
-        bool pair_ok = EXT && fast && !pz;
-        if (EXT) {
+        // EXT: sort the thread's trials by c, largest first (so x_0 >= x_1 >= ... for every point: dt2 >= 0 and RN is
+        // monotone), remember which trial sits in which slot, and check how far apart the phases get over the light curve
+        int org[R];  // trial (0..R-1, relative to s0) held by slot r
 #pragma unroll
-            for (int w2 = 0; w2 < RW; ++w2) {
-                const int e = 2 * w2, o = (2 * w2 + 1) % R;
-                swp[w2] = cc[e] < cc[o];
-                if (swp[w2]) {
-                    const double tc = cc[e]; cc[e] = cc[o]; cc[o] = tc;
-                    const int64_t tq = qv[e]; qv[e] = qv[o]; qv[o] = tq;
-                    const bool tv = valid[e]; valid[e] = valid[o]; valid[o] = tv;
+        for (int r = 0; r < R; ++r) org[r] = r;
+        bool pair_ok = EXT && fast && !pz, quad_ok = pair_ok;
+        if (EXT) {
+            auto cswap = [&](const int i, const int j) {  // compare-exchange: afterwards cc[i] >= cc[j]
+                if (cc[i] < cc[j]) {
+                    const double tc = cc[i]; cc[i] = cc[j]; cc[j] = tc;
+                    const int64_t tq = qv[i]; qv[i] = qv[j]; qv[j] = tq;
+                    const bool tv = valid[i]; valid[i] = valid[j]; valid[j] = tv;
+                    const int to = org[i]; org[i] = org[j]; org[j] = to;
                 }
-                pair_ok = pair_ok && ((cc[e] - cc[o]) * dt_max * dt_max < 0.999);
-            }
+            };
+            if (R == 4) { cswap(0, 1 % R); cswap(2 % R, 3 % R); cswap(0, 2 % R); cswap(1 % R, 3 % R); cswap(1 % R, 2 % R); }
+            else cswap(0, 1 % R);
+            const double d2 = dt_max * dt_max;
+#pragma unroll
+            for (int w2 = 0; w2 < RW; ++w2) pair_ok = pair_ok && ((cc[2 * w2] - cc[(2 * w2 + 1) % R]) * d2 < 0.999);
+            quad_ok = quad_ok && ((cc[0] - cc[R - 1]) * d2 < 0.999);
             pair_ok = __all_sync(0xffffffffu, pair_ok);
+            quad_ok = __all_sync(0xffffffffu, quad_ok);
         }
 
         int64_t S2[R];
@@ -372,9 +383,10 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-                        if (pz) fold_range<R, SHARE_P, true, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-                        else fold_range<R, SHARE_P, false, false>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        if (pz) fold_range<R, SHARE_P, true, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        else fold_range<R, SHARE_P, false, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
                     } else {
                         fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, inc0, inc1);
                     }
@@ -460,9 +472,16 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
             if (prm.out_ce) {
                 const int64_t o = (int64_t)lc * prm.n_trials + s0;  // q == slot outside DUMP
                 float *o32 = reinterpret_cast<float *>(prm.out_ce) + o;
-                double cet[R];  // CE in trial order (EXT may have swapped the slots of a pair)
+                double cet[R];  // CE in trial order (EXT has sorted the slots by c)
 #pragma unroll
-                for (int r = 0; r < R; ++r) cet[r] = (EXT && swp[r >> 1]) ? ce[(r ^ 1) % R] : ce[r];
+                for (int t = 0; t < R; ++t) {
+                    cet[t] = ce[t];
+                    if (EXT) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r)
+                            if (org[r] == t) cet[t] = ce[r];
+                    }
+                }
                 if (R == 4 && !prm.ce_fp64 && s0 + R <= prm.n_trials && (reinterpret_cast<uintptr_t>(o32) & 15u) == 0) {
                     *reinterpret_cast<float4 *>(o32) = make_float4((float)cet[0], (float)cet[1 % R], (float)cet[2 % R], (float)cet[3 % R]);
                 } else {
