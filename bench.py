@@ -45,10 +45,10 @@ FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (DESIG
 N_SM = 148
 OVERLAP = [False]   # set from --overlap; the oracle legs time the same binning
 # DRAM traffic of one k_search launch from the committed ncu --set full capture (profiles/r1_k_search_C3_full.md):
-# C3: 15.9 MB read + 774.0 MB written (the algorithmic output is the 819.2 MB fp32 cube; part of it is still in L2 at
+# C3: 15.6 MB read + 772.0 MB written (the algorithmic output is the 819.2 MB fp32 cube; part of it is still in L2 at
 # kernel end); C5 (profiles/r1_k_search_C5_full.md, no cube): 2.5 MB read, 256 B written.  Only workloads that were
 # captured have an entry.
-NCU_DRAM_BYTES_PER_LAUNCH = {"C3": 15.9e6 + 774.0e6, "C5": 2.5e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"C3": 15.6e6 + 772.0e6, "C5": 2.5e6}
 
 
 def load_peaks():
