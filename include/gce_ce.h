@@ -19,7 +19,9 @@
  *     NULL = default stream) and return without synchronising; results are valid once the stream has
  *     reached that point.  gce_ce_search_host synchronises before returning.
  *   - Return value: 0 (GCE_CE_OK) = enqueued; negative = error and nothing was enqueued.
- *   - No global mutable state; re-entrant across streams as long as each call has its own workspace.
+ *   - No global mutable state on the device-pointer calls; re-entrant across streams as long as each call has its
+ *     own workspace.  The *_host entry points allocate from a library-private, thread-safe memory pool per device
+ *     that keeps up to 1 GiB cached between calls; gce_ce_host_release() returns it to the driver.
  *   - `times` need not be sorted.  `periods` are in the unit of `times`; `pdots` are dimensionless (s/s), any
  *     sign (:228).  Trials are addressed by the flat index q = ip * n_pdot + ipd.
  *   - Values that need device data to validate (non-monotone lc_offsets, P <= 0, non-finite inputs, a light
@@ -129,6 +131,9 @@ int gce_ce_merge_partials(const int64_t *partials, int32_t n_parts, int32_t n_lc
  * one GPU first, then one blob array per GPU over the interconnect). */
 int gce_ce_merge_partials_to_partial(const int64_t *partials, int32_t n_parts, int32_t n_lc,
                                      const gce_ce_params *prm_host, int64_t *out_partial, void *stream);
+
+/* Returns the cached device memory of the *_host entry points to the driver (see Conventions). */
+int gce_ce_host_release(void);
 
 /* Test-only: the production search kernel run in "dump" mode over a list of flat trial indices
  * (device int64[n_trials], the same list for every light curve); writes the histogram counts

@@ -53,13 +53,13 @@ _lib.gce_ce_strerror.restype = C.c_char_p
 _lib.gce_ce_version.restype = C.c_char_p
 for _f in ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
            "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_last_cuda_error",
-           "gce_ce_search_partial", "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial"):
+           "gce_ce_search_partial", "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release"):
     getattr(_lib, _f).restype = C.c_int
 
 EXPORTS = ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
            "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_strerror",
            "gce_ce_last_cuda_error", "gce_ce_version", "gce_ce_partial_words", "gce_ce_search_partial",
-           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial")
+           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release")
 
 
 class GceError(RuntimeError):
@@ -146,6 +146,12 @@ def gce_ce_search(times, mags, lc_offsets, periods, pdots, prm: Params, out_ce=N
                               periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), _ptr(out_ce),
                               _ptr(out_best_idx), _ptr(out_best_ce), _ptr(out_stats), _ptr(workspace),
                               workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def gce_ce_host_release() -> None:
+    """Return the cached device memory of the host entry points to the driver."""
+    _lib.gce_ce_host_release.restype = C.c_int
+    _check(_lib.gce_ce_host_release())
 
 
 def gce_ce_partial_words(top_k) -> int:

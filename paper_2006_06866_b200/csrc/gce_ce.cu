@@ -492,6 +492,43 @@ int gce_ce_validate_host(const double *times, const double *mags, const int64_t 
     return GCE_CE_OK;
 }
 
+// Device memory of the host-buffer entry points comes from a library-private stream-ordered pool per device whose
+// release threshold keeps up to 1 GiB cached between calls (the default pool hands everything back to the driver at
+// every synchronisation, which costs 20 - 200 ms per call for a few hundred MB).  gce_ce_host_release() trims it.
+static cudaMemPool_t g_host_pool[64] = {};
+static std::mutex g_host_pool_mutex;
+
+static cudaError_t host_pool(cudaMemPool_t *pool) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_host_pool_mutex);
+    if (!g_host_pool[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        e = cudaMemPoolCreate(&g_host_pool[dev], &props);
+        if (e != cudaSuccess) { g_host_pool[dev] = nullptr; return e; }
+        uint64_t keep = 1ull << 30;
+        cudaMemPoolSetAttribute(g_host_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    *pool = g_host_pool[dev];
+    return cudaSuccess;
+}
+
+int gce_ce_host_release(void) {
+    std::lock_guard<std::mutex> lock(g_host_pool_mutex);
+    for (int d = 0; d < 64; ++d)
+        if (g_host_pool[d]) {
+            cudaError_t e = cudaMemPoolTrimTo(g_host_pool[d], 0);
+            if (e != cudaSuccess) return cuda_fail(e);
+        }
+    return GCE_CE_OK;
+}
+
 // Host-buffer entry with the cube requested and a grid worth splitting: the period axis is cut into chunks searched
 // back to back on one stream (gce_ce_search_partial, exact merge at the end) while a second stream copies each finished
 // cube slice to the caller's buffer, so the device-to-host transfer of the cube overlaps the search of the next chunk.
@@ -505,9 +542,12 @@ static int search_host_pipelined(const double *times, const double *mags, const 
     size_t ws_bytes = 0;
     int rc = gce_ce_workspace_bytes(total, n_lc, chunk, n_pdot, prm, &ws_bytes);
     if (rc) return rc;
+    cudaMemPool_t pool = nullptr;
+    cudaError_t e = host_pool(&pool);
+    if (e != cudaSuccess) return cuda_fail(e);
     cudaStream_t st = nullptr, st2 = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
-    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
     if (e != cudaSuccess) return cuda_fail(e);
     e = cudaStreamCreateWithFlags(&st2, cudaStreamNonBlocking);
     if (e != cudaSuccess) { cudaStreamDestroy(st); return cuda_fail(e); }
@@ -517,7 +557,7 @@ static int search_host_pipelined(const double *times, const double *mags, const 
     }
     void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
     void *d_sl[2] = {nullptr, nullptr}, *d_part = nullptr, *d_idx = nullptr, *d_bce = nullptr, *d_st = nullptr;
-    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocAsync(p, bytes ? bytes : 16, st); };
+    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st); };
     const size_t slice_bytes = (size_t)n_lc * (size_t)chunk * (size_t)n_pdot * esz;
     rc = GCE_CE_OK;
     do {
@@ -600,12 +640,15 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
     const size_t ce_bytes = out_ce ? (size_t)n_lc * n_trials * (prm->ce_fp64 ? 8 : 4) : 0;
     const size_t k = (size_t)prm->top_k;
 
+    cudaMemPool_t pool = nullptr;
+    cudaError_t e = host_pool(&pool);
+    if (e != cudaSuccess) return cuda_fail(e);
     cudaStream_t st;
-    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
     if (e != cudaSuccess) return cuda_fail(e);
     void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
     void *d_ce = nullptr, *d_idx = nullptr, *d_bce = nullptr, *d_st = nullptr;
-    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocAsync(p, bytes ? bytes : 16, st); };
+    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st); };
     rc = GCE_CE_OK;
     do {
         if ((e = dalloc(&d_t, 8 * (size_t)total)) || (e = dalloc(&d_m, 8 * (size_t)total)) ||
