@@ -19,8 +19,9 @@
 // one RED.shared per point-fold; the phase marginal lives in registers (compile-time n_phi) and the entropy is
 // accumulated in 2^-42 fixed point so CE does not depend on summation order.  The phase bin is
 // floor(y) - n_phi * floor(x) from two round-down magic adds (exact for |y| < 2^51, no integer division: on sm_100
-// IMAD.HI is quarter rate and slows the FP64 pipe, measured in DESIGN.md section 7).  No tensor cores: this is a
-// histogram/entropy path, not a contraction.
+// IMAD.HI is quarter rate and slows the FP64 pipe, measured in DESIGN.md section 7); where the shared memory allows
+// 2 n_phi + 1 counter rows, the trials of a thread share one floor(x) (gce_search.cuh, "MODE 1 / 2").  No tensor
+// cores: this is a histogram/entropy path, not a contraction.
 //
 // This translation unit must be compiled with -fmad=false; the fold additionally uses explicit _rn/_rd
 // intrinsics, which are never contracted.

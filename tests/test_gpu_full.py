@@ -347,3 +347,26 @@ def test_pair_floor_variant_matches_oracle(gce, oracle, n_phi, pdots):
     torch.cuda.synchronize()
     assert_ce_close(res32.ce.cpu().numpy(), ref, RTOL32)
     assert torch.equal(res32.best_idx, res.best_idx)
+
+
+def test_pair_floor_variant_streams_a_long_light_curve(gce, oracle):
+    """The extended-row variant is planned from the AVERAGE light-curve length; one light curve that is longer than the
+    remaining shared-memory buffer (3420 points beside 168 KB of counters) is streamed through two half buffers."""
+    rng = np.random.default_rng(17)
+    lcs = []
+    for n in [300] * 11 + [6001]:
+        t = np.sort(rng.uniform(0, 9e7, n))
+        lcs.append((t, W.two_dip_mags(rng, t, 533.0, -4e-11, 0.5, 0.2, 0.05)))
+    times = np.concatenate([t for t, _ in lcs]); mags = np.concatenate([m for _, m in lcs])
+    offs = np.cumsum([0] + [t.size for t, _ in lcs]).astype(np.int64)
+    periods = 1.0 / np.linspace(1 / 1200.0, 1 / 400.0, 520)
+    pdots = np.linspace(-8e-11, 0.0, 8)
+    ref = oracle.ce_search(times, mags, offs, periods, pdots, 20, 10)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(times), d(mags), d(offs), d(periods), d(pdots), 20, 10, top_k=3, want_cube=True, ce_fp64=True,
+                     want_stats=True)
+    torch.cuda.synchronize()
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    for lc in range(12):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 3, RTOL64, oracle)
+    np.testing.assert_allclose(res.stats.cpu().numpy(), _stats_ref(oracle, ref.reshape(12, -1)), rtol=RTOL_STATS)
