@@ -478,7 +478,7 @@ int gce_ce_validate_host(const double *times, const double *mags, const int64_t 
     if (lc_offsets[0] != 0) return GCE_CE_ERR_RANGE;
     for (int32_t l = 0; l < n_lc; ++l) {
         const int64_t n = lc_offsets[l + 1] - lc_offsets[l];
-        if (n < 0 || n > GCE_CE_MAX_POINTS) return GCE_CE_ERR_RANGE;
+        if (n < 0 || n > (prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS)) return GCE_CE_ERR_RANGE;
     }
     const int64_t total = lc_offsets[n_lc];
     if (total > 0 && (!times || !mags)) return GCE_CE_ERR_POINTER;
