@@ -370,3 +370,37 @@ def test_pair_floor_variant_streams_a_long_light_curve(gce, oracle):
     for lc in range(12):
         assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 3, RTOL64, oracle)
     np.testing.assert_allclose(res.stats.cpu().numpy(), _stats_ref(oracle, ref.reshape(12, -1)), rtol=RTOL_STATS)
+
+
+@pytest.mark.parametrize("n_phi,overlap,step", [(20, False, 0.30), (20, False, 0.45), (20, False, 3.0), (15, False, 0.30),
+                                                (50, True, 0.33), (50, False, 0.6), (50, True, 5.0)])
+def test_pdot_zero_grids_fine_and_coarse(gce, oracle, n_phi, overlap, step):
+    """Pdot = {0} on frequency grids from properly oversampled (step x 1/T between neighbouring trials; the paper uses
+    1/(3T)) to coarse, with the paper's VRO-like time sampling: the trials of a thread have different
+    periods (no shared a = dt/P, no shared floors).  (Sharing floors between neighbouring periods was measured: +5 % on
+    this kind of grid, -2 to -10 % on every BASELINE config through the larger kernels, so it is not built.)"""
+    rng = np.random.default_rng(23)
+    lcs = []
+    for n in (500, 731, 64):
+        t = W.vro_like_cadence(rng, n)
+        lcs.append((t, W.two_dip_mags(rng, t, 1234.5, 0.0, 0.4, 0.2, 0.1)))
+    times = np.concatenate([t for t, _ in lcs]); mags = np.concatenate([m for _, m in lcs])
+    offs = np.cumsum([0] + [t.size for t, _ in lcs]).astype(np.int64)
+    T = max(float(t[-1]) for t, _ in lcs)
+    freqs = 1 / 1500.0 + (step / T) * np.arange(3001)
+    periods = np.ascontiguousarray(1.0 / freqs)
+    n_m = 10 if n_phi != 15 else 8
+    ref = oracle.ce_search(times, mags, offs, periods, np.zeros(1), n_phi, n_m, overlap=overlap)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(times), d(mags), d(offs), d(periods), d(np.zeros(1)), n_phi, n_m, top_k=3, want_cube=True,
+                     ce_fp64=True, want_stats=True, overlap=overlap)
+    torch.cuda.synchronize()
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    for lc in range(3):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 3, RTOL64, oracle)
+    np.testing.assert_allclose(res.stats.cpu().numpy(), _stats_ref(oracle, ref.reshape(3, -1)), rtol=RTOL_STATS)
+    # ascending periods (descending 1/P) give the same cube, reversed
+    res_r = gce.search(d(times), d(mags), d(offs), d(periods[::-1].copy()), d(np.zeros(1)), n_phi, n_m, top_k=0,
+                       want_cube=True, ce_fp64=True, overlap=overlap)
+    torch.cuda.synchronize()
+    assert torch.equal(res_r.ce.flip(1), res.ce)
