@@ -1,0 +1,78 @@
+"""Seeded differential test of the CUDA path against the oracle over random shapes: bin counts 1..64, 1..9 Pdot values of
+either sign, ragged batches incl. empty and very short light curves, plain / overlapping bins, fp32 / fp64 cubes, top-k
+0..32, Eq. 5 on and off.  Every kernel variant (R = 2 / 4, shared or distinct periods, compile-time and generic n_phi,
+register and shared-memory marginals, shared floors) is reached by some case."""
+import numpy as np
+import pytest
+import torch
+
+import gce_workloads as W
+from test_gpu_parity import RTOL32, RTOL64, assert_ce_close, assert_topk_matches
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gce():
+    from paper_2006_06866_b200.build import build
+    build()
+    import paper_2006_06866_b200 as g
+    return g
+
+
+def _case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    n_phi = int(rng.choice([1, 2, 3, 7, 15, 20, 30, 50, 64, int(rng.integers(1, 65))]))
+    n_m = int(rng.choice([1, 2, 8, 10, 64, int(rng.integers(1, 65))]))
+    n_pdot = int(rng.choice([1, 1, 2, 3, 4, 4, 8, 9]))
+    n_p = int(rng.integers(1, 700))
+    n_lc = int(rng.integers(1, 6))
+    lens = rng.choice([0, 1, 2, 5, 40, 333, 1200, 2500], size=n_lc)
+    lcs = []
+    for n in lens:
+        t = np.sort(rng.uniform(0.0, rng.choice([1e5, 3e7, 2e8]), size=int(n))) + rng.choice([0.0, 5e8])
+        m = rng.normal(size=int(n)) if rng.random() < 0.8 else np.round(rng.normal(size=int(n)), 1)   # ties on bin edges
+        lcs.append((t, m))
+    times = np.concatenate([t for t, _ in lcs]) if lcs else np.zeros(0)
+    mags = np.concatenate([m for _, m in lcs]) if lcs else np.zeros(0)
+    offs = np.cumsum([0] + [t.size for t, _ in lcs]).astype(np.int64)
+    p_lo, p_hi = sorted(rng.uniform(60.0, 20000.0, size=2))
+    periods = np.ascontiguousarray(1.0 / np.linspace(1.0 / p_hi, 1.0 / p_lo, n_p))
+    scale = 10.0 ** rng.uniform(-13, -8)
+    pdots = np.zeros(1) if (n_pdot == 1 and rng.random() < 0.6) else rng.uniform(-scale, scale * rng.choice([0.0, 0.3]), n_pdot)
+    if rng.random() < 0.5:
+        pdots = np.sort(pdots)
+    overlap = bool(rng.random() < 0.35)
+    top_k = int(rng.choice([0, 1, 3, 5, 32]))
+    return dict(times=times, mags=mags, offs=offs, periods=periods, pdots=np.ascontiguousarray(pdots), n_phi=n_phi, n_m=n_m,
+                overlap=overlap, top_k=top_k, fp64=bool(rng.random() < 0.6), stats=bool(rng.random() < 0.5))
+
+
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("GCE_FUZZ_N", "48"))))
+def test_random_shapes_match_oracle(gce, oracle, seed):
+    c = _case(seed)
+    ref = oracle.ce_search(c["times"], c["mags"], c["offs"], c["periods"], c["pdots"], c["n_phi"], c["n_m"],
+                           overlap=c["overlap"])
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    res = gce.search(d(c["times"]), d(c["mags"]), d(c["offs"]), d(c["periods"]), d(c["pdots"]), c["n_phi"], c["n_m"],
+                     top_k=c["top_k"], want_cube=True, ce_fp64=c["fp64"], want_stats=c["stats"], overlap=c["overlap"])
+    torch.cuda.synchronize()
+    rtol = RTOL64 if c["fp64"] else RTOL32
+    assert_ce_close(res.ce.cpu().numpy(), ref, rtol)
+    n_lc = c["offs"].size - 1
+    if c["top_k"]:
+        for lc in range(n_lc):
+            assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), c["top_k"], rtol,
+                                oracle)
+    if c["stats"]:
+        st = res.stats.cpu().numpy()
+        for lc in range(n_lc):
+            row = ref[lc].ravel()
+            if c["offs"][lc + 1] == c["offs"][lc]:
+                assert np.all(np.isnan(st[lc]))
+                continue
+            assert st[lc, 0] == pytest.approx(row.mean(), rel=1e-9, abs=1e-13)
+            assert st[lc, 2] == pytest.approx(row.min(), rel=1e-9, abs=1e-13)
+            sd = row.std()
+            if sd > 1e-9 * max(abs(row.mean()), 1e-300):
+                assert st[lc, 1] == pytest.approx(sd, rel=1e-7)
