@@ -9,7 +9,7 @@
  * Written from /root/reference/PAPER.md (Katz et al., arXiv 2006.06866):
  *   - magnitude normalisation            PAPER.md:96   (reading Q2 of DESIGN.md: min/max -> [0,1])
  *   - phase fold with Pdot, Eq. 3
- *   - 2-D phase x magnitude histogram     PAPER.md:106  (non-overlapping bins; reading Q3)
+ *   - 2-D phase x magnitude histogram     PAPER.md:106  (non-overlapping bins; the 50 %-overlapping variant: reading Q3)
  *   - conditional entropy, Eq. 4
  *   - minimum CE = best (P, Pdot)
  *   - significance, Eq. 5
