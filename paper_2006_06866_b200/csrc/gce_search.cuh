@@ -58,7 +58,7 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
                                              const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0, const uint32_t inc1) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
-    if (MODE != 0) {
+    if constexpr (MODE != 0) {
         static_assert(MODE == 0 || (SHARE_P && !PZ && R % 2 == 0), "shared floors need one period and Pdot != 0");
         double x[R];
 #pragma unroll
@@ -76,17 +76,17 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
                 red_add_u32(Iy * rs + base, h ? inc1 : inc0);
             }
         }
-        return;
-    }
+    } else {
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
-        const double x = PZ ? a : __dadd_rn(a, __dmul_rn(p.y, cc[r]));
-        const double y = __dmul_rn(x, nphi_d);
-        const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
-        const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
-        const uint32_t j = Iy + Ix * negn;
-        red_add_u32(j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
+        for (int r = 0; r < R; ++r) {
+            if (!SHARE_P) a = __dmul_rn(p.x, invP[r]);
+            const double x = PZ ? a : __dadd_rn(a, __dmul_rn(p.y, cc[r]));
+            const double y = __dmul_rn(x, nphi_d);
+            const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
+            const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
+            const uint32_t j = Iy + Ix * negn;
+            red_add_u32(j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
+        }
     }
 }
 
