@@ -101,7 +101,7 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
         if (nt_s > kMaxThreadsSmemMarg) nt_s = kMaxThreadsSmemMarg;
         p.nt = (int)nt_s;  // >= 32: 64 x 64 bins with R = 4 leave room for 192 threads
     }
-    p.nphi_t = templ ? n_phi : 0;
+    p.nphi_t = (templ && p.regm) ? n_phi : 0;  // compile-time n_phi kernels exist with register marginals only
     // extended rows (one FP64 instruction fewer per two point-folds, C3: 83 -> 77 ms): instantiated for n_phi = 15 and
     // 20 with R = 4 trials sharing a period; taken when the whole average light curve still fits beside the counters
     p.ext = p.regm && p.share_p && p.R == 4 && (n_phi == 15 || n_phi == 20) && n_pdot > 1 &&
@@ -211,14 +211,12 @@ int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t
         return launch_search<20, true, 4, true, false, true>(sp, plan, n_lc, st);
     }
     switch (plan.nphi_t) {
-        case 15: return plan.regm ? launch_search_variant<15, true>(sp, plan, n_lc, st) : launch_search_variant<15, false>(sp, plan, n_lc, st);
-        case 20: return plan.regm ? launch_search_variant<20, true>(sp, plan, n_lc, st) : launch_search_variant<20, false>(sp, plan, n_lc, st);
-        case 30: return plan.regm ? launch_search_variant<30, true>(sp, plan, n_lc, st) : launch_search_variant<30, false>(sp, plan, n_lc, st);
-        case 50:
-            if (plan.regm && plan.R == 2)
-                return plan.share_p ? launch_search<50, true, 2, true, false>(sp, plan, n_lc, st)
-                                    : launch_search<50, true, 2, false, false>(sp, plan, n_lc, st);
-            return launch_search_variant<0, false>(sp, plan, n_lc, st);
+        case 15: return launch_search_variant<15, true>(sp, plan, n_lc, st);
+        case 20: return launch_search_variant<20, true>(sp, plan, n_lc, st);
+        case 30: return launch_search_variant<30, true>(sp, plan, n_lc, st);
+        case 50:  // make_plan: R == 2
+            return plan.share_p ? launch_search<50, true, 2, true, false>(sp, plan, n_lc, st)
+                                : launch_search<50, true, 2, false, false>(sp, plan, n_lc, st);
         default: return launch_search_variant<0, false>(sp, plan, n_lc, st);
     }
 }
