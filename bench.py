@@ -240,7 +240,7 @@ def run_ours(args):
     bce = torch.empty((w.n_lc, k), dtype=torch.float32, device=dev) if k else None
     ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, w.n_p, w.n_pdot, prm), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    launches_per_step = gce.gce_ce_launch_count(w.n_lc, prm)
+    launches_per_step = gce.gce_ce_launch_count(w.n_lc, w.n_p, prm)
 
     def step():
         gce.gce_ce_search(times, mags, offs, periods, pdots, prm, ce, bidx, bce, None, ws)

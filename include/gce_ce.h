@@ -18,14 +18,20 @@
  *   - gce_ce_search and the debug calls only enqueue work on `stream` (a cudaStream_t passed as void*,
  *     NULL = default stream) and return without synchronising; results are valid once the stream has
  *     reached that point.  gce_ce_search_host synchronises before returning.
- *   - Return value: 0 (GCE_CE_OK) = enqueued; negative = error and nothing was enqueued.
+ *   - Return value: 0 (GCE_CE_OK) = enqueued.  Negative = error: argument, size, plan and workspace checks all
+ *     run before the first launch, so for every code except GCE_CE_ERR_CUDA nothing was enqueued; after
+ *     GCE_CE_ERR_CUDA (a launch or event record failed) the outputs are undefined.
  *   - No global mutable state on the device-pointer calls; re-entrant across streams as long as each call has its
  *     own workspace.  The *_host entry points allocate from a library-private, thread-safe memory pool per device
  *     that keeps up to 1 GiB cached between calls; gce_ce_host_release() returns it to the driver.
  *   - `times` need not be sorted.  `periods` are in the unit of `times`; `pdots` are dimensionless (s/s), any
  *     sign (:228).  Trials are addressed by the flat index q = ip * n_pdot + ipd.
- *   - Values that need device data to validate (non-monotone lc_offsets, P <= 0, non-finite inputs, a light
- *     curve longer than GCE_CE_MAX_POINTS) are undefined behaviour; gce_ce_validate_host checks host copies.
+ *   - Values that need device data to validate (non-monotone lc_offsets, P <= 0, non-finite inputs) are
+ *     undefined behaviour on the device-pointer calls; gce_ce_validate_host checks host copies.  A light curve
+ *     longer than GCE_CE_MAX_POINTS (GCE_CE_MAX_POINTS_OVERLAP with overlap = 1) is never folded with wrapped
+ *     counters: the device-pointer calls return GCE_CE_ERR_RANGE when total_points alone proves it and
+ *     otherwise treat that light curve as empty (CE = NaN, best index -1); the *_host calls, which see the
+ *     offsets, return GCE_CE_ERR_RANGE.
  *   - A light curve with N = 0 yields CE = NaN for every trial and best index -1; N = 1 yields CE = 0.
  *   - There is no CPU fallback anywhere in this library.
  */
@@ -135,10 +141,14 @@ int gce_ce_merge_partials_to_partial(const int64_t *partials, int32_t n_parts, i
 /* Returns the cached device memory of the *_host entry points to the driver (see Conventions). */
 int gce_ce_host_release(void);
 
-/* Test-only: the production search kernel run in "dump" mode over a list of flat trial indices
- * (device int64[n_trials], the same list for every light curve); writes the histogram counts
- *   out_counts uint32[n_lc][n_trials][n_phase_bins][n_mag_bins]      (phase-major, as Eq. 4's n_ij)
- * and, if out_ce_at != NULL, double[n_lc][n_trials] CE of those trials. */
+/* Test-only: the search kernel gce_ce_search would launch for this grid -- same plan, same instantiation compiled in
+ * dump mode, same tiles, warps and fold modes -- restricted to the tiles that hold a listed trial.  trial_q is a device
+ * list int64[n_trials] of distinct flat trial indices q = ip * n_pdot + ipd of the (n_p x n_pdot) grid, the same for
+ * every light curve.  Writes the count table Eq. 4 is evaluated on,
+ *   out_counts uint32[n_lc][n_trials][n_phase_bins][n_mag_bins]      (phase-major, n_ij; with prm->overlap = 1 the
+ *                                                                     overlapped table c[k][i] = n[k][i] + n[k-1][i])
+ * and, if out_ce_at != NULL, double[n_lc][n_trials] CE of those trials.  Workspace as for gce_ce_workspace_bytes(
+ * total_points, n_lc, n_p, n_pdot, prm).  top_k and want_stats are ignored. */
 int gce_ce_debug_histogram(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                            int64_t total_points, const double *periods, int64_t n_p, const double *pdots,
                            int64_t n_pdot, const gce_ce_params *prm_host, const int64_t *trial_q,
@@ -146,11 +156,21 @@ int gce_ce_debug_histogram(const double *times, const double *mags, const int64_
                            size_t workspace_bytes, void *stream);
 
 /* Test-only: phase bin and magnitude bin of every point of light curve `lc` for trial q, in the caller's
- * point order: out_phase_bin int32[N], out_mag_bin int32[N]. */
+ * point order: out_phase_bin int32[N], out_mag_bin int32[N].  The bins come from the search kernel's own fold
+ * functions, called with the thread context the search builds for trial q (its R - 1 slot neighbours, slots sorted by
+ * c where floors can be shared).  fold_mode selects which of the kernel's fold variants runs: GCE_CE_FOLD_AUTO = the one
+ * the owning thread qualifies for, or one of them forced; out_fold_mode (device int32[1], may be NULL) receives the
+ * variant used, or -1 -- and every bin is -1 -- when the forced variant's precondition does not hold for this trial. */
+#define GCE_CE_FOLD_AUTO 0
+#define GCE_CE_FOLD_PLAIN 1     /* j = floor(y) - n_phi floor(x), one floor(x) per trial; needs |y| < 2^51        */
+#define GCE_CE_FOLD_PAIR 2      /* the two trials of a counter word share floor(x); needs them within one cycle  */
+#define GCE_CE_FOLD_QUAD 3      /* all trials of the thread share floor(x); needs them within one cycle          */
+#define GCE_CE_FOLD_GENERIC 4   /* 64-bit integer floor and modulus, any |y| < 2^62                              */
+#define GCE_CE_FOLD_PDOT_ZERO 5 /* every c of the thread is +-0: x = a                                           */
 int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                       const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                      const gce_ce_params *prm_host, int32_t lc, int64_t q, int32_t *out_phase_bin,
-                      int32_t *out_mag_bin, void *stream);
+                      const gce_ce_params *prm_host, int32_t lc, int64_t q, int32_t fold_mode,
+                      int32_t *out_phase_bin, int32_t *out_mag_bin, int32_t *out_fold_mode, void *stream);
 
 /* Synchronous argument checker on HOST copies of the arrays (the hot call never synchronises).
  * Returns GCE_CE_OK or the first error found. */
@@ -158,8 +178,9 @@ int gce_ce_validate_host(const double *times_host, const double *mags_host, cons
                          int32_t n_lc, const double *periods_host, int64_t n_p, const double *pdots_host,
                          int64_t n_pdot, const gce_ce_params *prm_host);
 
-/* Number of kernels one gce_ce_search call enqueues for these arguments (for launch accounting). */
-int gce_ce_launch_count(int32_t n_lc, const gce_ce_params *prm_host);
+/* Number of kernels one gce_ce_search (partial = 0) or gce_ce_search_partial (partial = 1) call over n_p periods
+ * enqueues for these arguments (for launch accounting). */
+int gce_ce_launch_count(int32_t n_lc, int64_t n_p, const gce_ce_params *prm_host, int partial);
 
 const char *gce_ce_strerror(int code);
 int gce_ce_last_cuda_error(void); /* cudaError_t of the most recent GCE_CE_ERR_CUDA on this thread */

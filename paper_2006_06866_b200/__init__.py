@@ -1,7 +1,7 @@
 """gce-b200: Conditional Entropy (P, Pdot) period search for NVIDIA B200 (sm_100a).
 
 The product is the C-ABI library declared in include/gce_ce.h (built in-tree as libgce_ce.so from
-csrc/gce_ce.cu); this package is its ctypes binding.  The binding is loaded on first use of any of its
+csrc/gce_ce.cu and csrc/gce_search_family.cu); this package is its ctypes binding.  The binding is loaded on first use of any of its
 names and raises ImportError if the library has not been built -- there is no CPU fallback.  Build with
 `python -m paper_2006_06866_b200.build` (the build module itself must be importable before the library
 exists, hence the lazy load).

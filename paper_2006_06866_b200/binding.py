@@ -22,6 +22,7 @@ _lib = C.CDLL(LIB)
 
 MAX_BINS, MAX_TOPK, MAX_POINTS = 64, 32, 65535
 OK, ERR_POINTER, ERR_RANGE, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
+FOLD_AUTO, FOLD_PLAIN, FOLD_PAIR, FOLD_QUAD, FOLD_GENERIC, FOLD_PDOT_ZERO = range(6)   # gce_ce_debug_bins fold_mode
 
 
 class Params(C.Structure):
@@ -37,8 +38,8 @@ _lib.gce_ce_search.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, 
 _lib.gce_ce_search_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _vp, _vp, _vp, _vp]
 _lib.gce_ce_debug_histogram.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params),
                                         _vp, _i64, _vp, _vp, _vp, _sz, _vp]
-_lib.gce_ce_debug_bins.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _i32, _i64,
-                                   _vp, _vp, _vp]
+_lib.gce_ce_debug_bins.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _i32, _i64, _i32,
+                                   _vp, _vp, _vp, _vp]
 _lib.gce_ce_partial_words.argtypes = [_i32]
 _lib.gce_ce_partial_words.restype = _sz
 _lib.gce_ce_search_partial.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params), _i64, _i64,
@@ -47,7 +48,7 @@ _lib.gce_ce_merge_partials.argtypes = [_vp, _i32, _i32, C.POINTER(Params), _vp, 
 _lib.gce_ce_merge_partials_to_partial.argtypes = [_vp, _i32, _i32, C.POINTER(Params), _vp, _vp]
 _lib.gce_ce_merge_partials_to_partial.restype = C.c_int
 _lib.gce_ce_validate_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params)]
-_lib.gce_ce_launch_count.argtypes = [_i32, C.POINTER(Params)]
+_lib.gce_ce_launch_count.argtypes = [_i32, _i64, C.POINTER(Params), C.c_int]
 _lib.gce_ce_strerror.argtypes = [C.c_int]
 _lib.gce_ce_strerror.restype = C.c_char_p
 _lib.gce_ce_version.restype = C.c_char_p
@@ -96,8 +97,8 @@ def gce_ce_workspace_bytes(total_points, n_lc, n_p, n_pdot, prm: Params) -> int:
     return int(out.value)
 
 
-def gce_ce_launch_count(n_lc, prm: Params) -> int:
-    return int(_lib.gce_ce_launch_count(int(n_lc), C.byref(prm)))
+def gce_ce_launch_count(n_lc, n_p, prm: Params, partial=False) -> int:
+    return int(_lib.gce_ce_launch_count(int(n_lc), int(n_p), C.byref(prm), int(bool(partial))))
 
 
 def _dev(t, dtype):
@@ -198,6 +199,7 @@ def gce_ce_merge_partials(partials, n_parts, n_lc, prm: Params, out_best_idx=Non
 
 def gce_ce_debug_histogram(times, mags, lc_offsets, periods, pdots, prm: Params, trial_q, out_counts, out_ce_at=None,
                            workspace=None, stream=None):
+    """The search kernel of this grid in dump mode: count tables (and CE) of the listed flat trials."""
     n_lc = lc_offsets.numel() - 1
     _dev(trial_q, torch.int64)
     _dev(out_counts, torch.int32)  # uint32 counts viewed as int32 storage
@@ -212,13 +214,15 @@ def gce_ce_debug_histogram(times, mags, lc_offsets, periods, pdots, prm: Params,
 
 
 def gce_ce_debug_bins(times, mags, lc_offsets, periods, pdots, prm: Params, lc, q, out_phase_bin, out_mag_bin,
-                      stream=None):
+                      fold_mode=FOLD_AUTO, out_fold_mode=None, stream=None):
     n_lc = lc_offsets.numel() - 1
     _dev(out_phase_bin, torch.int32)
     _dev(out_mag_bin, torch.int32)
+    if out_fold_mode is not None:
+        _dev(out_fold_mode, torch.int32)
     _check(_lib.gce_ce_debug_bins(_ptr(times), _ptr(mags), _ptr(lc_offsets), n_lc, _ptr(periods), periods.numel(),
-                                  _ptr(pdots), pdots.numel(), C.byref(prm), int(lc), int(q), _ptr(out_phase_bin),
-                                  _ptr(out_mag_bin), _stream(stream)))
+                                  _ptr(pdots), pdots.numel(), C.byref(prm), int(lc), int(q), int(fold_mode),
+                                  _ptr(out_phase_bin), _ptr(out_mag_bin), _ptr(out_fold_mode), _stream(stream)))
 
 
 def _host(a, dtype):

@@ -2,7 +2,7 @@
 //
 // Path (citations are PAPER.md lines of arXiv 2006.06866):
 //   k_preprocess  S1  t0 / min-max / magnitude bin per point, points grouped by magnitude bin      (:96)
-//   k_ltab            fixed-point table L(k) = k ln k used by S4
+//                     (+ the fixed-point table L(k) = k ln k used by S4, built by the same launch)
 //   k_search      S2  fp64 fold, Eq. 3, frozen operation order               (:100)
 //                 S3  per-trial private histogram in shared memory                                 (:106)
 //                 S4  N*CE = sum_j L(n_j) - sum_ij L(n_ij), exact integer accumulation, Eq. 4      (:108)
@@ -27,7 +27,7 @@
 // intrinsics, which are never contracted.
 #include "gce_common.cuh"
 #include "gce_preprocess.cuh"
-#include "gce_search.cuh"
+#include "gce_debug.cuh"
 #include "gce_select.cuh"
 
 namespace {
@@ -36,21 +36,6 @@ namespace {
 thread_local int g_last_cuda_error = 0;
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-
-// Which kernel variant runs, with how many threads, over how many CTAs: decided from sizes only (deterministic, no
-// device query), so gce_ce_workspace_bytes and gce_ce_search agree.
-struct Plan {
-    int R;             // trials per thread
-    bool share_p;      // the R trials of a thread share one period
-    int nphi_t;        // compile-time n_phi of the kernel (15, 20, 30) or 0 = generic
-    bool regm;         // phase marginal in registers (512 threads) instead of shared memory
-    bool ext;          // 2 n_phi + 1 counter rows: the two trials of a counter word share one floor(x) (gce_search.cuh)
-    int nt;            // threads per CTA (multiple of 32)
-    int cap_points;    // shared-memory point buffer capacity
-    size_t smem;       // dynamic shared memory per CTA
-    int64_t tiles_per_lc;
-    int jobs_per_lc;
-};
 
 constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-marginal kernels (<= 102 registers)
 constexpr int kMinPoints = 640;           // smallest point buffer; also the top-k merge scratch (16 B x 20 warps x 32)
@@ -66,17 +51,21 @@ size_t search_smem_per_thread(int n_phi, int R, bool regm, bool ext = false) {
     return (size_t)((R + 1) / 2) * (size_t)(regm ? hist_rows : hist_rows + n_phi) * sizeof(uint32_t);
 }
 
-Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_pdot, int n_phi, bool dump) {
-    Plan p;
-    if (dump) { p.R = 2; p.share_p = false; }
-    else if (n_pdot % 4 == 0) { p.R = 4; p.share_p = true; }
-    else if (n_pdot % 2 == 0) { p.R = 2; p.share_p = true; }
-    else { p.R = 4; p.share_p = false; }
-    const int64_t avail = (int64_t)kSmemLimit - (int64_t)search_smem_fixed();
-    const bool templ = !dump && (n_phi == 15 || n_phi == 20 || n_phi == 30 || n_phi == 50);
+// Trials per thread and whether they share a period: from the grid shape alone (also used by gce_ce_debug_bins).
+void plan_trials(int64_t n_pdot, int n_phi, int *R, bool *share_p) {
+    if (n_pdot % 4 == 0) { *R = 4; *share_p = true; }
+    else if (n_pdot % 2 == 0) { *R = 2; *share_p = true; }
+    else { *R = 4; *share_p = false; }
     // 50 phase bins (the paper's production binning): the register marginal of R = 4 trials would take
     // 100 registers, so a thread owns R = 2 trials and 512 threads still fit (measured 2x the generic variant)
-    if (!dump && n_phi == 50) { p.R = 2; p.share_p = (n_pdot % 2 == 0); }
+    if (n_phi == 50) { *R = 2; *share_p = (n_pdot % 2 == 0); }
+}
+
+Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_pdot, int n_phi) {
+    Plan p;
+    plan_trials(n_pdot, n_phi, &p.R, &p.share_p);
+    const int64_t avail = (int64_t)kSmemLimit - (int64_t)search_smem_fixed();
+    const bool templ = n_phi == 15 || n_phi == 20 || n_phi == 30 || n_phi == 50;
     // point buffer wanted: the average light curve plus a quarter (the per-LC lengths live on the device; a longer
     // light curve is streamed through the buffer in two halves instead of staying resident)
     const int64_t avg = n_lc > 0 ? (total_points + n_lc - 1) / n_lc : 0;
@@ -89,12 +78,12 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     };
     int64_t nt_s = threads_beside(want_pts, false);
     if (nt_s > kMaxThreadsSmemMarg) nt_s = kMaxThreadsSmemMarg;
-    const bool regm_fits = templ && threads_beside(kMinPoints, true) >= 512;
+    const bool regm_fits = templ && threads_beside(kMinPoints, true) >= kNtRegm;
     // measured on C3: 512 threads with register marginals beat 608 threads with shared-memory
     // marginals (83.7 vs 86.8 ms), so the register variant is taken whenever it fits
     if (regm_fits) {
         p.regm = true;
-        p.nt = 512;
+        p.nt = kNtRegm;
     } else {
         p.regm = false;
         if (nt_s < 32) nt_s = threads_beside(kMinPoints, false);
@@ -128,7 +117,7 @@ struct Layout {
     int ltab_n;
 };
 
-Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t n_pdot, const gce_ce_params *prm, bool dump) {
+Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t n_pdot, const gce_ce_params *prm) {
     Layout L;
     size_t o = 0;
     L.pts = o; o = align_up(o + sizeof(double2) * (size_t)(total_points > 0 ? total_points : 1), 256);
@@ -138,7 +127,7 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     if (tn > GCE_CE_MAX_POINTS) tn = GCE_CE_MAX_POINTS;
     L.ltab_n = (int)tn + 1;
     L.ltab = o; o = align_up(o + sizeof(int64_t) * (size_t)L.ltab_n, 256);
-    const Plan p = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins, dump);
+    const Plan p = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins);
     const size_t parts = (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc * (size_t)(prm->top_k > 0 ? prm->top_k : 1);
     L.part_S = o; o = align_up(o + sizeof(int64_t) * parts, 256);
     L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
@@ -167,17 +156,15 @@ int check_sizes(int32_t n_lc, int64_t total_points, int64_t n_p, int64_t n_pdot)
     return GCE_CE_OK;
 }
 
-// Exact 32-bit floor-mod constants: q = umulhi(I, M) equals I / d for I < nmax.
-void mod_constants(int d, uint32_t *mul, uint32_t *bias, double *y_safe) {
-    if (d == 1) { *mul = 0; *bias = 0; *y_safe = -1.0; return; }  // always the generic path (j = 0)
-    const uint64_t M = (1ULL << 32) / (uint64_t)d + 1;
-    const uint64_t e = M * (uint64_t)d - (1ULL << 32);
-    const uint64_t nmax = 0xffffffffULL / e;
-    const uint64_t half = nmax / 2;
-    const uint64_t B = half / (uint64_t)d * (uint64_t)d;
-    *mul = (uint32_t)M;
-    *bias = (uint32_t)B;
-    *y_safe = (double)(B - (uint64_t)d - 2);
+// Light-curve lengths from a HOST copy of lc_offsets: non-negative and within the counter range.
+int check_lengths_host(const int64_t *lc_offsets, int32_t n_lc, const gce_ce_params *prm) {
+    if (n_lc > 0 && lc_offsets[0] != 0) return GCE_CE_ERR_RANGE;
+    const int64_t lim = prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS;
+    for (int32_t l = 0; l < n_lc; ++l) {
+        const int64_t n = lc_offsets[l + 1] - lc_offsets[l];
+        if (n < 0 || n > lim) return GCE_CE_ERR_RANGE;
+    }
+    return GCE_CE_OK;
 }
 
 int cuda_fail(cudaError_t e) {
@@ -185,40 +172,17 @@ int cuda_fail(cudaError_t e) {
     return GCE_CE_ERR_CUDA;
 }
 
-template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT = false>
-int launch_search(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
-    auto kern = k_search<NPHI, REGM, R, SHARE_P, DUMP, EXT>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem);
-    if (e != cudaSuccess) return cuda_fail(e);
-    const unsigned grid = (unsigned)((int64_t)n_lc * plan.jobs_per_lc);
-    kern<<<grid, plan.nt, plan.smem, st>>>(sp);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e);
-    return GCE_CE_OK;
-}
-
-template <int NPHI, bool REGM>
-int launch_search_variant(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
-    if (plan.share_p && plan.R == 4) return launch_search<NPHI, REGM, 4, true, false>(sp, plan, n_lc, st);
-    if (plan.share_p && plan.R == 2) return launch_search<NPHI, REGM, 2, true, false>(sp, plan, n_lc, st);
-    return launch_search<NPHI, REGM, 4, false, false>(sp, plan, n_lc, st);
-}
-
 int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t n_lc, cudaStream_t st) {
-    if (dump) return launch_search<0, false, 2, false, true>(sp, plan, n_lc, st);
-    if (plan.ext) {  // make_plan: regm, share_p, R == 4, n_phi 15 or 20
-        if (plan.nphi_t == 15) return launch_search<15, true, 4, true, false, true>(sp, plan, n_lc, st);
-        return launch_search<20, true, 4, true, false, true>(sp, plan, n_lc, st);
-    }
+    cudaError_t e = cudaErrorInvalidValue;
     switch (plan.nphi_t) {
-        case 15: return launch_search_variant<15, true>(sp, plan, n_lc, st);
-        case 20: return launch_search_variant<20, true>(sp, plan, n_lc, st);
-        case 30: return launch_search_variant<30, true>(sp, plan, n_lc, st);
-        case 50:  // make_plan: R == 2
-            return plan.share_p ? launch_search<50, true, 2, true, false>(sp, plan, n_lc, st)
-                                : launch_search<50, true, 2, false, false>(sp, plan, n_lc, st);
-        default: return launch_search_variant<0, false>(sp, plan, n_lc, st);
+        case 0: e = dump ? launch_search_n0_d1(sp, plan, n_lc, st) : launch_search_n0_d0(sp, plan, n_lc, st); break;
+        case 15: e = dump ? launch_search_n15_d1(sp, plan, n_lc, st) : launch_search_n15_d0(sp, plan, n_lc, st); break;
+        case 20: e = dump ? launch_search_n20_d1(sp, plan, n_lc, st) : launch_search_n20_d0(sp, plan, n_lc, st); break;
+        case 30: e = dump ? launch_search_n30_d1(sp, plan, n_lc, st) : launch_search_n30_d0(sp, plan, n_lc, st); break;
+        case 50: e = dump ? launch_search_n50_d1(sp, plan, n_lc, st) : launch_search_n50_d0(sp, plan, n_lc, st); break;
+        default: break;
     }
+    return e == cudaSuccess ? GCE_CE_OK : cuda_fail(e);
 }
 
 }  // namespace
@@ -226,13 +190,13 @@ int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t
 // ================================================================================================ C ABI
 extern "C" {
 
-const char *gce_ce_version(void) { return "gce-b200 0.1 (sm_100a)"; }
+const char *gce_ce_version(void) { return "gce-b200 0.2 (sm_100a)"; }
 
 const char *gce_ce_strerror(int code) {
     switch (code) {
         case GCE_CE_OK: return "ok";
         case GCE_CE_ERR_POINTER: return "null or inconsistent pointer arguments";
-        case GCE_CE_ERR_RANGE: return "size, bin count or option out of range";
+        case GCE_CE_ERR_RANGE: return "size, bin count, light-curve length or option out of range";
         case GCE_CE_ERR_WORKSPACE: return "workspace too small or misaligned";
         case GCE_CE_ERR_CUDA: return "CUDA runtime error (see gce_ce_last_cuda_error)";
         default: return "unknown error code";
@@ -241,9 +205,10 @@ const char *gce_ce_strerror(int code) {
 
 int gce_ce_last_cuda_error(void) { return g_last_cuda_error; }
 
-int gce_ce_launch_count(int32_t n_lc, const gce_ce_params *prm) {
+int gce_ce_launch_count(int32_t n_lc, int64_t n_p, const gce_ce_params *prm, int partial) {
     if (!prm || n_lc <= 0) return 0;
-    return 3 + (prm->top_k > 0 ? 1 : 0) + (prm->want_stats ? 1 : 0);  // ltab, preprocess, search, [merge_topk], [merge_stats]
+    // preprocess (+ table), search (when the grid is not empty), [merge_topk], [merge_stats: Eq. 5 and every partial blob]
+    return 1 + (n_p > 0 ? 1 : 0) + (prm->top_k > 0 ? 1 : 0) + ((prm->want_stats || partial) ? 1 : 0);
 }
 
 int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int64_t n_pdot, const gce_ce_params *prm,
@@ -253,10 +218,12 @@ int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int6
     if (rc) return rc;
     rc = check_sizes(n_lc, total_points, n_p, n_pdot);
     if (rc) return rc;
-    *bytes = make_layout(total_points, n_lc, n_p * n_pdot, n_pdot, prm, false).total;
+    *bytes = make_layout(total_points, n_lc, n_p * n_pdot, n_pdot, prm).total;
     return GCE_CE_OK;
 }
 
+// Every fallible host-side step (argument, plan and workspace checks) comes before the first launch; after that only a
+// failing launch or event record can return an error, and then the outputs are undefined.
 static int run_search(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                       int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
                       const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce, double *out_stats,
@@ -273,7 +240,8 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     if (n_p > 0 && !periods) return GCE_CE_ERR_POINTER;
     if (!pdots) return GCE_CE_ERR_POINTER;
     if (dump) {
-        if (!trial_q || n_dump < 0) return GCE_CE_ERR_POINTER;
+        if (n_dump < 0 || n_dump > 0x7fffffff) return GCE_CE_ERR_RANGE;
+        if (n_dump > 0 && !trial_q) return GCE_CE_ERR_POINTER;
     } else {
         if (out_partial) {
             if (out_best_idx || out_best_ce || out_stats) return GCE_CE_ERR_POINTER;
@@ -284,11 +252,12 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
             if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
         }
     }
-    const int64_t n_trials = dump ? n_dump : n_p * n_pdot;
-    gce_ce_params lay_prm = *prm;
-    if (dump) { lay_prm.top_k = 0; lay_prm.want_stats = 0; lay_prm.overlap = 0; }  // the debug dump is always the plain table
-    const int mult = lay_prm.overlap ? 2 : 1;
-    const Layout L = make_layout(total_points, n_lc, n_trials, dump ? 1 : n_pdot, &lay_prm, dump);
+    // more points than every light curve could hold within the counter range: some light curve must be too long
+    const int64_t max_points = prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS;
+    if (total_points > (int64_t)n_lc * max_points) return GCE_CE_ERR_RANGE;
+    const int64_t n_trials = n_p * n_pdot;
+    const int mult = prm->overlap ? 2 : 1;
+    const Layout L = make_layout(total_points, n_lc, n_trials, n_pdot, prm);
     if (workspace_bytes < L.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return GCE_CE_ERR_WORKSPACE;
     if (n_lc == 0) return GCE_CE_OK;
 
@@ -299,20 +268,13 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     LcInfo *info = reinterpret_cast<LcInfo *>(ws + L.info);
     int64_t *ltab = reinterpret_cast<int64_t *>(ws + L.ltab);
 
-    k_ltab<<<(L.ltab_n + 255) / 256, 256, 0, st>>>(ltab, L.ltab_n);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e);
-    k_preprocess<<<n_lc, 256, 0, st>>>(times, mags, lc_offsets, prm->n_mag_bins, pts, seg, info, ltab, mult);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e);
-
-    const Plan plan = make_plan(n_lc, total_points, n_trials, dump ? 1 : n_pdot, prm->n_phase_bins, dump);
+    const Plan plan = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins);
     SearchParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.pts = pts; sp.seg = seg; sp.info = info; sp.lc_offsets = lc_offsets; sp.ltab = ltab;
-    sp.periods = periods; sp.pdots = pdots; sp.trial_q = trial_q;
+    sp.periods = periods; sp.pdots = pdots; sp.trial_q = trial_q; sp.n_dump = n_dump;
     sp.n_p = n_p; sp.n_pdot = n_pdot; sp.n_trials = n_trials;
-    sp.q_off = dump ? 0 : ip_begin * n_pdot;
+    sp.q_off = ip_begin * n_pdot;
     sp.jobs_per_lc = plan.jobs_per_lc;
     sp.tiles_per_lc = plan.tiles_per_lc;
     sp.cap_points = plan.cap_points;
@@ -320,18 +282,22 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.ltab_n = L.ltab_n;
     sp.top_k = dump ? 0 : prm->top_k;
     sp.ce_fp64 = prm->ce_fp64;
-    sp.overlap = lay_prm.overlap;
+    sp.overlap = prm->overlap;
     sp.out_ce = out_ce;
     sp.part_S = reinterpret_cast<int64_t *>(ws + L.part_S);
     sp.part_q = reinterpret_cast<int64_t *>(ws + L.part_q);
     sp.part_stats = (!dump && prm->want_stats) ? reinterpret_cast<uint64_t *>(ws + L.part_stats) : nullptr;
     sp.out_counts = out_counts; sp.out_ce_at = out_ce_at;
 
+    k_preprocess<<<n_lc + (L.ltab_n + 255) / 256, 256, 0, st>>>(times, mags, lc_offsets, n_lc, prm->n_mag_bins, pts, seg, info,
+                                                              ltab, L.ltab_n, mult, (int)max_points);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
     if (prm->ev_search_begin) {
         e = cudaEventRecord(reinterpret_cast<cudaEvent_t>(prm->ev_search_begin), st);
         if (e != cudaSuccess) return cuda_fail(e);
     }
-    if (n_trials > 0) {
+    if (n_trials > 0 && !(dump && n_dump == 0)) {
         rc = dispatch_search(sp, plan, dump, n_lc, st);
         if (rc) return rc;
     }
@@ -450,17 +416,26 @@ int gce_ce_debug_histogram(const double *times, const double *mags, const int64_
 
 int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                       const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot, const gce_ce_params *prm,
-                      int32_t lc, int64_t q, int32_t *out_phase_bin, int32_t *out_mag_bin, void *stream) {
+                      int32_t lc, int64_t q, int32_t fold_mode, int32_t *out_phase_bin, int32_t *out_mag_bin,
+                      int32_t *out_fold_mode, void *stream) {
     int rc = check_params(prm);
     if (rc) return rc;
     if (!times || !mags || !lc_offsets || !periods || !pdots || !out_phase_bin || !out_mag_bin) return GCE_CE_ERR_POINTER;
     if (n_pdot < 1 || n_p < 1 || lc < 0 || lc >= n_lc || q < 0 || q >= n_p * n_pdot) return GCE_CE_ERR_RANGE;
-    uint32_t mul, bias;
-    double y_safe;
-    mod_constants(prm->n_phase_bins, &mul, &bias, &y_safe);
-    k_debug_bins<<<1, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(times, mags, lc_offsets, periods, pdots, n_pdot,
-                                                                       prm->n_phase_bins, prm->n_mag_bins, lc, q, mul,
-                                                                       bias, y_safe, out_phase_bin, out_mag_bin);
+    if (fold_mode < GCE_CE_FOLD_AUTO || fold_mode > GCE_CE_FOLD_PDOT_ZERO) return GCE_CE_ERR_RANGE;
+    int R;
+    bool share_p;
+    plan_trials(n_pdot, prm->n_phase_bins, &R, &share_p);
+    SearchParams sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.periods = periods; sp.pdots = pdots;
+    sp.n_p = n_p; sp.n_pdot = n_pdot; sp.n_trials = n_p * n_pdot;
+    sp.n_phi = prm->n_phase_bins; sp.n_m = prm->n_mag_bins;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (R == 4 && share_p) k_debug_bins<4, true><<<1, 256, 0, st>>>(times, mags, lc_offsets, sp, lc, q, fold_mode, out_phase_bin, out_mag_bin, out_fold_mode);
+    else if (R == 2 && share_p) k_debug_bins<2, true><<<1, 256, 0, st>>>(times, mags, lc_offsets, sp, lc, q, fold_mode, out_phase_bin, out_mag_bin, out_fold_mode);
+    else if (R == 4) k_debug_bins<4, false><<<1, 256, 0, st>>>(times, mags, lc_offsets, sp, lc, q, fold_mode, out_phase_bin, out_mag_bin, out_fold_mode);
+    else k_debug_bins<2, false><<<1, 256, 0, st>>>(times, mags, lc_offsets, sp, lc, q, fold_mode, out_phase_bin, out_mag_bin, out_fold_mode);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return GCE_CE_OK;
@@ -474,10 +449,8 @@ int gce_ce_validate_host(const double *times, const double *mags, const int64_t 
     if (!lc_offsets) return GCE_CE_ERR_POINTER;
     if (n_lc < 0 || n_p < 0 || n_pdot < 1) return GCE_CE_ERR_RANGE;
     if (lc_offsets[0] != 0) return GCE_CE_ERR_RANGE;
-    for (int32_t l = 0; l < n_lc; ++l) {
-        const int64_t n = lc_offsets[l + 1] - lc_offsets[l];
-        if (n < 0 || n > (prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS)) return GCE_CE_ERR_RANGE;
-    }
+    rc = check_lengths_host(lc_offsets, n_lc, prm);
+    if (rc) return rc;
     const int64_t total = lc_offsets[n_lc];
     if (total > 0 && (!times || !mags)) return GCE_CE_ERR_POINTER;
     for (int64_t k = 0; k < total; ++k)
@@ -509,10 +482,13 @@ static cudaError_t host_pool(cudaMemPool_t *pool) {
         props.handleTypes = cudaMemHandleTypeNone;
         props.location.type = cudaMemLocationTypeDevice;
         props.location.id = dev;
-        e = cudaMemPoolCreate(&g_host_pool[dev], &props);
-        if (e != cudaSuccess) { g_host_pool[dev] = nullptr; return e; }
+        cudaMemPool_t mp = nullptr;
+        e = cudaMemPoolCreate(&mp, &props);
+        if (e != cudaSuccess) return e;
         uint64_t keep = 1ull << 30;
-        cudaMemPoolSetAttribute(g_host_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+        e = cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) { cudaMemPoolDestroy(mp); return e; }
+        g_host_pool[dev] = mp;
     }
     *pool = g_host_pool[dev];
     return cudaSuccess;
@@ -528,6 +504,40 @@ int gce_ce_host_release(void) {
     return GCE_CE_OK;
 }
 
+// Streams, events and pool allocations of one host-entry call; everything is released by the destructor, whatever path
+// the call leaves on.  CU(x): run a CUDA call, on failure record it and leave the do { } while (0) block.
+namespace {
+struct HostCall {
+    cudaMemPool_t pool = nullptr;
+    cudaStream_t st = nullptr, st2 = nullptr;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    void *mem[16] = {};
+    int n_mem = 0;
+    cudaError_t alloc(void **p, size_t bytes) {
+        cudaError_t e = cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st);
+        if (e == cudaSuccess) mem[n_mem++] = *p;
+        return e;
+    }
+    ~HostCall() {
+        if (st2) cudaStreamSynchronize(st2);
+        for (int i = 0; i < n_mem; ++i) cudaFreeAsync(mem[i], st);
+        if (st) cudaStreamSynchronize(st);
+        for (cudaEvent_t e : ev)
+            if (e) cudaEventDestroy(e);
+        if (st2) cudaStreamDestroy(st2);
+        if (st) cudaStreamDestroy(st);
+    }
+};
+}  // namespace
+#define CU(x)                                   \
+    {                                           \
+        const cudaError_t cu_e_ = (x);          \
+        if (cu_e_ != cudaSuccess) {             \
+            rc = cuda_fail(cu_e_);              \
+            break;                              \
+        }                                       \
+    }
+
 // Host-buffer entry with the cube requested and a grid worth splitting: the period axis is cut into chunks searched
 // back to back on one stream (gce_ce_search_partial, exact merge at the end) while a second stream copies each finished
 // cube slice to the caller's buffer, so the device-to-host transfer of the cube overlaps the search of the next chunk.
@@ -541,55 +551,52 @@ static int search_host_pipelined(const double *times, const double *mags, const 
     size_t ws_bytes = 0;
     int rc = gce_ce_workspace_bytes(total, n_lc, chunk, n_pdot, prm, &ws_bytes);
     if (rc) return rc;
-    cudaMemPool_t pool = nullptr;
-    cudaError_t e = host_pool(&pool);
-    if (e != cudaSuccess) return cuda_fail(e);
-    cudaStream_t st = nullptr, st2 = nullptr;
-    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
-    e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
-    if (e != cudaSuccess) return cuda_fail(e);
-    e = cudaStreamCreateWithFlags(&st2, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { cudaStreamDestroy(st); return cuda_fail(e); }
-    for (int b = 0; b < 2; ++b) {
-        cudaEventCreateWithFlags(&ev_done[b], cudaEventDisableTiming);
-        cudaEventCreateWithFlags(&ev_free[b], cudaEventDisableTiming);
-    }
+    HostCall hc;
     void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
     void *d_sl[2] = {nullptr, nullptr}, *d_part = nullptr, *d_idx = nullptr, *d_bce = nullptr, *d_st = nullptr;
-    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st); };
     const size_t slice_bytes = (size_t)n_lc * (size_t)chunk * (size_t)n_pdot * esz;
-    rc = GCE_CE_OK;
     do {
-        if ((e = dalloc(&d_t, 8 * (size_t)total)) || (e = dalloc(&d_m, 8 * (size_t)total)) ||
-            (e = dalloc(&d_off, 8 * (size_t)(n_lc + 1))) || (e = dalloc(&d_p, 8 * (size_t)n_p)) ||
-            (e = dalloc(&d_pd, 8 * (size_t)n_pdot)) || (e = dalloc(&d_ws, ws_bytes)) ||
-            (e = dalloc(&d_sl[0], slice_bytes)) || (e = dalloc(&d_sl[1], slice_bytes)) ||
-            (e = dalloc(&d_part, 8 * W * (size_t)n_lc * (size_t)n_chunks)) || (e = dalloc(&d_idx, 8 * (size_t)n_lc * k)) ||
-            (e = dalloc(&d_bce, 4 * (size_t)n_lc * k)) || (e = dalloc(&d_st, 32 * (size_t)n_lc))) { rc = cuda_fail(e); break; }
-        cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(d_p, periods, 8 * (size_t)n_p, cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st);
+        CU(host_pool(&hc.pool));
+        CU(cudaStreamCreateWithFlags(&hc.st, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&hc.st2, cudaStreamNonBlocking));
+        bool ev_ok = true;
+        for (int i = 0; i < 4 && ev_ok; ++i) {
+            const cudaError_t e = cudaEventCreateWithFlags(&hc.ev[i], cudaEventDisableTiming);
+            if (e != cudaSuccess) { rc = cuda_fail(e); ev_ok = false; }
+        }
+        if (!ev_ok) break;
+        cudaEvent_t *ev_done = hc.ev, *ev_free = hc.ev + 2;
+        cudaStream_t st = hc.st, st2 = hc.st2;
+        CU(hc.alloc(&d_t, 8 * (size_t)total)); CU(hc.alloc(&d_m, 8 * (size_t)total));
+        CU(hc.alloc(&d_off, 8 * (size_t)(n_lc + 1))); CU(hc.alloc(&d_p, 8 * (size_t)n_p));
+        CU(hc.alloc(&d_pd, 8 * (size_t)n_pdot)); CU(hc.alloc(&d_ws, ws_bytes));
+        CU(hc.alloc(&d_sl[0], slice_bytes)); CU(hc.alloc(&d_sl[1], slice_bytes));
+        CU(hc.alloc(&d_part, 8 * W * (size_t)n_lc * (size_t)n_chunks)); CU(hc.alloc(&d_idx, 8 * (size_t)n_lc * k));
+        CU(hc.alloc(&d_bce, 4 * (size_t)n_lc * k)); CU(hc.alloc(&d_st, 32 * (size_t)n_lc));
+        CU(cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_p, periods, 8 * (size_t)n_p, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st));
         int n_done = 0;
         for (int c = 0; c < n_chunks && rc == GCE_CE_OK; ++c) {
             const int64_t a = (int64_t)c * chunk, b = a + chunk < n_p ? a + chunk : n_p;
             if (a >= b) break;
             const int buf = c & 1;
-            if (c >= 2) cudaStreamWaitEvent(st, ev_free[buf], 0);  // the copy that last read this slice buffer is done
+            cudaError_t e = cudaSuccess;
+            if (c >= 2) e = cudaStreamWaitEvent(st, ev_free[buf], 0);  // the copy that last read this slice buffer is done
+            if (e != cudaSuccess) { rc = cuda_fail(e); break; }
             rc = gce_ce_search_partial((const double *)d_t, (const double *)d_m, (const int64_t *)d_off, n_lc, total,
                                        (const double *)d_p, n_p, (const double *)d_pd, n_pdot, prm, a, b, d_sl[buf],
                                        (int64_t *)d_part + (size_t)c * (size_t)n_lc * W, d_ws, ws_bytes, st);
             if (rc) break;
             ++n_done;
-            cudaEventRecord(ev_done[buf], st);
-            cudaStreamWaitEvent(st2, ev_done[buf], 0);
             const size_t width = (size_t)(b - a) * (size_t)n_pdot * esz;  // one light curve's rows of this slice
-            e = cudaMemcpy2DAsync(static_cast<unsigned char *>(out_ce) + (size_t)a * (size_t)n_pdot * esz,
-                                  (size_t)n_p * (size_t)n_pdot * esz, d_sl[buf], width, width, (size_t)n_lc,
-                                  cudaMemcpyDeviceToHost, st2);
-            if (e != cudaSuccess) { rc = cuda_fail(e); break; }
-            cudaEventRecord(ev_free[buf], st2);
+            if ((e = cudaEventRecord(ev_done[buf], st)) != cudaSuccess || (e = cudaStreamWaitEvent(st2, ev_done[buf], 0)) != cudaSuccess ||
+                (e = cudaMemcpy2DAsync(static_cast<unsigned char *>(out_ce) + (size_t)a * (size_t)n_pdot * esz,
+                                       (size_t)n_p * (size_t)n_pdot * esz, d_sl[buf], width, width, (size_t)n_lc,
+                                       cudaMemcpyDeviceToHost, st2)) != cudaSuccess ||
+                (e = cudaEventRecord(ev_free[buf], st2)) != cudaSuccess) { rc = cuda_fail(e); break; }
         }
         if (rc) break;
         if (k || prm->want_stats) {
@@ -597,20 +604,12 @@ static int search_host_pipelined(const double *times, const double *mags, const 
                                        out_best_ce ? (float *)d_bce : nullptr, out_stats ? (double *)d_st : nullptr, st);
             if (rc) break;
         }
-        if (out_best_idx && k) cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
-        if (out_best_ce && k) cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
-        if (out_stats) cudaMemcpyAsync(out_stats, d_st, 32 * (size_t)n_lc, cudaMemcpyDeviceToHost, st);
+        if (out_best_idx && k) CU(cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st));
+        if (out_best_ce && k) CU(cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st));
+        if (out_stats) CU(cudaMemcpyAsync(out_stats, d_st, 32 * (size_t)n_lc, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st2));
+        CU(cudaStreamSynchronize(st));
     } while (0);
-    e = cudaStreamSynchronize(st2);
-    if (e != cudaSuccess && rc == GCE_CE_OK) rc = cuda_fail(e);
-    void *frees[] = {d_t, d_m, d_off, d_p, d_pd, d_ws, d_sl[0], d_sl[1], d_part, d_idx, d_bce, d_st};
-    for (void *p : frees)
-        if (p) cudaFreeAsync(p, st);
-    e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess && rc == GCE_CE_OK) rc = cuda_fail(e);
-    for (int b = 0; b < 2; ++b) { cudaEventDestroy(ev_done[b]); cudaEventDestroy(ev_free[b]); }
-    cudaStreamDestroy(st2);
-    cudaStreamDestroy(st);
     return rc;
 }
 
@@ -624,6 +623,11 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
     const int64_t total = lc_offsets[n_lc];
     rc = check_sizes(n_lc, total, n_p, n_pdot);
     if (rc) return rc;
+    rc = check_lengths_host(lc_offsets, n_lc, prm);  // the host entry sees the offsets: a checked error, not NaN
+    if (rc) return rc;
+    if (total > 0 && (!times || !mags)) return GCE_CE_ERR_POINTER;
+    if ((n_p > 0 && !periods) || !pdots) return GCE_CE_ERR_POINTER;
+    if (!out_ce && !out_best_idx && !out_stats) return GCE_CE_ERR_POINTER;
     if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
     if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
     if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
@@ -639,47 +643,38 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
     const size_t ce_bytes = out_ce ? (size_t)n_lc * n_trials * (prm->ce_fp64 ? 8 : 4) : 0;
     const size_t k = (size_t)prm->top_k;
 
-    cudaMemPool_t pool = nullptr;
-    cudaError_t e = host_pool(&pool);
-    if (e != cudaSuccess) return cuda_fail(e);
-    cudaStream_t st;
-    e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
-    if (e != cudaSuccess) return cuda_fail(e);
+    HostCall hc;
     void *d_t = nullptr, *d_m = nullptr, *d_off = nullptr, *d_p = nullptr, *d_pd = nullptr, *d_ws = nullptr;
     void *d_ce = nullptr, *d_idx = nullptr, *d_bce = nullptr, *d_st = nullptr;
-    auto dalloc = [&](void **p, size_t bytes) { return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st); };
-    rc = GCE_CE_OK;
     do {
-        if ((e = dalloc(&d_t, 8 * (size_t)total)) || (e = dalloc(&d_m, 8 * (size_t)total)) ||
-            (e = dalloc(&d_off, 8 * (size_t)(n_lc + 1))) || (e = dalloc(&d_p, 8 * (size_t)n_p)) ||
-            (e = dalloc(&d_pd, 8 * (size_t)n_pdot)) || (e = dalloc(&d_ws, ws_bytes)) ||
-            (e = dalloc(&d_ce, ce_bytes)) || (e = dalloc(&d_idx, 8 * (size_t)n_lc * k)) ||
-            (e = dalloc(&d_bce, 4 * (size_t)n_lc * k)) || (e = dalloc(&d_st, 32 * (size_t)n_lc))) { rc = cuda_fail(e); break; }
+        CU(host_pool(&hc.pool));
+        CU(cudaStreamCreateWithFlags(&hc.st, cudaStreamNonBlocking));
+        cudaStream_t st = hc.st;
+        CU(hc.alloc(&d_t, 8 * (size_t)total)); CU(hc.alloc(&d_m, 8 * (size_t)total));
+        CU(hc.alloc(&d_off, 8 * (size_t)(n_lc + 1))); CU(hc.alloc(&d_p, 8 * (size_t)n_p));
+        CU(hc.alloc(&d_pd, 8 * (size_t)n_pdot)); CU(hc.alloc(&d_ws, ws_bytes));
+        CU(hc.alloc(&d_ce, ce_bytes)); CU(hc.alloc(&d_idx, 8 * (size_t)n_lc * k));
+        CU(hc.alloc(&d_bce, 4 * (size_t)n_lc * k)); CU(hc.alloc(&d_st, 32 * (size_t)n_lc));
         if (total) {
-            cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
-            cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st);
+            CU(cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
+            CU(cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
         }
-        cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st);
-        if (n_p) cudaMemcpyAsync(d_p, periods, 8 * (size_t)n_p, cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st);
+        CU(cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st));
+        if (n_p) CU(cudaMemcpyAsync(d_p, periods, 8 * (size_t)n_p, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_pd, pdots, 8 * (size_t)n_pdot, cudaMemcpyHostToDevice, st));
         rc = gce_ce_search((const double *)d_t, (const double *)d_m, (const int64_t *)d_off, n_lc, total,
                            (const double *)d_p, n_p, (const double *)d_pd, n_pdot, prm, out_ce ? d_ce : nullptr,
                            out_best_idx ? (int64_t *)d_idx : nullptr, out_best_ce ? (float *)d_bce : nullptr,
                            out_stats ? (double *)d_st : nullptr, d_ws, ws_bytes, st);
         if (rc) break;
-        if (out_ce && ce_bytes) cudaMemcpyAsync(out_ce, d_ce, ce_bytes, cudaMemcpyDeviceToHost, st);
-        if (out_best_idx && k) cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
-        if (out_best_ce && k) cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st);
-        if (out_stats && n_lc) cudaMemcpyAsync(out_stats, d_st, 32 * (size_t)n_lc, cudaMemcpyDeviceToHost, st);
+        if (out_ce && ce_bytes) CU(cudaMemcpyAsync(out_ce, d_ce, ce_bytes, cudaMemcpyDeviceToHost, st));
+        if (out_best_idx && k && n_lc) CU(cudaMemcpyAsync(out_best_idx, d_idx, 8 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st));
+        if (out_best_ce && k && n_lc) CU(cudaMemcpyAsync(out_best_ce, d_bce, 4 * (size_t)n_lc * k, cudaMemcpyDeviceToHost, st));
+        if (out_stats && n_lc) CU(cudaMemcpyAsync(out_stats, d_st, 32 * (size_t)n_lc, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
     } while (0);
-    void *frees[] = {d_t, d_m, d_off, d_p, d_pd, d_ws, d_ce, d_idx, d_bce, d_st};
-    for (void *p : frees)
-        if (p) cudaFreeAsync(p, st);
-    e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess && rc == GCE_CE_OK) rc = cuda_fail(e);
-    cudaStreamDestroy(st);
     return rc;
 }
+#undef CU
 
 }  // extern "C"
-

@@ -1,5 +1,5 @@
 // gce_common.cuh -- constants, shared structs, TMA / mbarrier helpers, warp top-k, Eq. 5 integer sums, frozen fold arithmetic
-// Part of the single translation unit gce_ce.cu (compiled with -fmad=false); see the header comment there.
+// Included by every translation unit of the library (all compiled with -fmad=false); see the header comment of gce_ce.cu.
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -10,21 +10,8 @@
 
 #include "gce_ce.h"
 
-namespace {
-
-
-constexpr int kLtabSmem = 1024;   // entries of the L table mirrored in shared memory
-constexpr int kLfixShift = 42;    // L table fixed point: 2^-42
-constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(y) in the low mantissa word
-constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
-constexpr int64_t kInfS = INT64_MAX;
-constexpr int kSmemLimit = 227 * 1024 - 8 * kLtabSmem;  // dynamic shared memory per CTA: 227 KB minus the static L table
-constexpr int kStatWords = 8;     // partial Eq. 5 sums: n, sum d (i128), sum d^2 (u192), min S, pad; d = S - K
-constexpr int kMaxWarps = 20;     // warps per CTA of the largest variant (640 threads)
-constexpr int kCloseGroup = 5;    // phase bins whose read-and-clear atomics are in flight together in S4
-
-struct FalseT { static constexpr bool value = false; };
-struct TrueT { static constexpr bool value = true; };
+// ---- types and entry points shared between the translation units (external linkage)
+namespace gce {
 
 struct LcInfo {
     int32_t n;
@@ -41,7 +28,8 @@ struct SearchParams {
     const int64_t *ltab;       // [ltab_n] fixed-point k ln k
     const double *periods;
     const double *pdots;
-    const int64_t *trial_q;    // DUMP only
+    const int64_t *trial_q;    // DUMP only: [n_dump] flat trial indices whose count tables are written out
+    int64_t n_dump;            // DUMP only
     int64_t n_p, n_pdot, n_trials;
     int64_t q_off;             // flat index of this call's first trial in the caller's grid (period sub-range)
     int64_t tiles_per_lc;
@@ -55,9 +43,60 @@ struct SearchParams {
     void *out_ce;              // cube or NULL
     int64_t *part_S, *part_q;  // [n_lc][jobs_per_lc][top_k]
     uint64_t *part_stats;      // [n_lc][jobs_per_lc][kStatWords] partial Eq. 5 sums, or NULL
-    uint32_t *out_counts;      // DUMP only
-    double *out_ce_at;         // DUMP only
+    uint32_t *out_counts;      // DUMP only: [n_lc][n_dump][n_phi][n_m]
+    double *out_ce_at;         // DUMP only: [n_lc][n_dump] or NULL
 };
+
+// Which kernel variant runs, with how many threads, over how many CTAs: decided from sizes only (deterministic, no
+// device query), so gce_ce_workspace_bytes, gce_ce_search and the debug dump agree.
+struct Plan {
+    int R;             // trials per thread
+    bool share_p;      // the R trials of a thread share one period
+    int nphi_t;        // compile-time n_phi of the kernel (15, 20, 30, 50) or 0 = generic
+    bool regm;         // phase marginal in registers instead of shared memory
+    bool ext;          // 2 n_phi + 1 counter rows: trials of a thread share one floor(x) (gce_search.cuh)
+    int nt;            // threads per CTA (multiple of 32)
+    int cap_points;    // shared-memory point buffer capacity
+    size_t smem;       // dynamic shared memory per CTA
+    int64_t tiles_per_lc;
+    int jobs_per_lc;
+};
+
+// One launcher per kernel family (compile-time n_phi) and mode, each in its own translation unit
+// (gce_search_family.cu compiled with -DGCE_FAMILY=<n_phi> -DGCE_DUMP=<0|1>) so that the build runs in parallel.
+// They pick the instantiation the plan names and launch it; cudaErrorInvalidValue if the plan names none.
+#define GCE_DECLARE_FAMILY(N)                                                                                  \
+    cudaError_t launch_search_n##N##_d0(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st); \
+    cudaError_t launch_search_n##N##_d1(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st);
+GCE_DECLARE_FAMILY(0)
+GCE_DECLARE_FAMILY(15)
+GCE_DECLARE_FAMILY(20)
+GCE_DECLARE_FAMILY(30)
+GCE_DECLARE_FAMILY(50)
+#undef GCE_DECLARE_FAMILY
+
+}  // namespace gce
+
+namespace {
+
+using namespace gce;
+
+constexpr int kLtabSmem = 1024;   // entries of the L table mirrored in shared memory
+constexpr int kLfixShift = 42;    // L table fixed point: 2^-42
+constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(y) in the low mantissa word
+constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
+constexpr int64_t kInfS = INT64_MAX;
+constexpr int kSmemLimit = 227 * 1024 - 8 * kLtabSmem;  // dynamic shared memory per CTA: 227 KB minus the static L table
+constexpr int kStatWords = 8;     // partial Eq. 5 sums: n, sum d (i128), sum d^2 (u192), min S, max S; d = S - K
+constexpr int kMaxWarps = 20;     // warps per CTA of the largest variant (640 threads)
+#ifndef GCE_NT_REGM
+#define GCE_NT_REGM 512
+#endif
+constexpr int kNtRegm = GCE_NT_REGM;  // threads per CTA of the register-marginal kernels (compile-time n_phi)
+constexpr int kCloseGroup = 5;    // phase bins whose read-and-clear atomics are in flight together in S4
+
+struct FalseT { static constexpr bool value = false; };
+struct TrueT { static constexpr bool value = true; };
 
 // ------------------------------------------------------------------------------------------------ helpers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {

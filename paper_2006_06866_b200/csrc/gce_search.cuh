@@ -52,10 +52,17 @@ __device__ __forceinline__ void ltab_pair(const int64_t *__restrict__ sL, const 
 // Then every j = floor(y) - n_phi * floor(x_base) lies in [0, 2 n_phi]; rows n_phi .. 2 n_phi are folded back (mod
 // n_phi) when the magnitude bin is closed.  Fewer FP64 instructions and one row-offset multiply-add per counter word
 // instead of per trial, the same bits.
-template <int R, bool SHARE_P, bool PZ, int MODE>
+// SINK receives (address of the counter word, slot r): the search kernel adds the slot's increment there with one RED
+// (RedSink); the per-point bin dump of gce_ce_debug_bins records the row instead (rs = 1, hb = 0: the address IS the row).
+struct RedSink {
+    uint32_t inc0, inc1;  // increments of the even / odd trial of a counter word (16-bit fields)
+    __device__ __forceinline__ void operator()(const uint32_t addr, const int r) const { red_add_u32(addr, (r & 1) ? inc1 : inc0); }
+};
+
+template <int R, bool SHARE_P, bool PZ, int MODE, typename SINK>
 __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
                                              const double nphi_d, const uint32_t negn, const uint32_t rs,
-                                             const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0, const uint32_t inc1) {
+                                             const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
     if constexpr (MODE != 0) {
@@ -73,7 +80,7 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
             for (int h = 0; h < 2; ++h) {
                 const double y = __dmul_rn(x[(r + h) % R], nphi_d);
                 const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
-                red_add_u32(Iy * rs + base, h ? inc1 : inc0);
+                sink(Iy * rs + base, r + h);
             }
         }
     } else {
@@ -85,46 +92,47 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
             const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
             const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
             const uint32_t j = Iy + Ix * negn;
-            red_add_u32(j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
+            sink(j * rs + hb[r >> 1], r);
         }
     }
 }
 
-template <int R, bool SHARE_P, bool PZ, int MODE>
+template <int R, bool SHARE_P, bool PZ, int MODE, typename SINK>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
-                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const uint32_t inc0,
-                                           const uint32_t inc1) {
+                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
     if (ke - kk >= 4) {
         double2 a0 = sp[kk], a1 = sp[kk + 1];
         do {
             const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-            fold_bin_add<R, SHARE_P, PZ, MODE>(a0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-            fold_bin_add<R, SHARE_P, PZ, MODE>(a1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(a0, invP, cc, nphi_d, negn, rs, hb, sink);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(a1, invP, cc, nphi_d, negn, rs, hb, sink);
             a0 = sp[kk + 4];
             a1 = sp[kk + 5];
-            fold_bin_add<R, SHARE_P, PZ, MODE>(b0, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-            fold_bin_add<R, SHARE_P, PZ, MODE>(b1, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(b0, invP, cc, nphi_d, negn, rs, hb, sink);
+            fold_bin_add<R, SHARE_P, PZ, MODE>(b1, invP, cc, nphi_d, negn, rs, hb, sink);
             kk += 4;
         } while (ke - kk >= 4);
     }
-    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE>(sp[kk], invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE>(sp[kk], invP, cc, nphi_d, negn, rs, hb, sink);
 }
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
-template <int R, bool SHARE_P>
+template <int R, bool SHARE_P, typename SINK>
+__device__ __forceinline__ void fold_bin_add_generic(const double2 p, const double (&invP)[R], const double (&cc)[R],
+                                                     const int n_phi, const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2],
+                                                     const SINK &sink) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
+        sink((uint32_t)j * rs + hb[r >> 1], r);
+    }
+}
+template <int R, bool SHARE_P, typename SINK>
 __device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ sp, int kk, const int ke,
                                                    const double (&invP)[R], const double (&cc)[R], const int n_phi,
-                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2],
-                                                   const uint32_t inc0, const uint32_t inc1) {
-    for (; kk < ke; ++kk) {
-        const double2 p = sp[kk];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
-            red_add_u32((uint32_t)j * rs + hb[r >> 1], (r & 1) ? inc1 : inc0);
-        }
-    }
+                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
+    for (; kk < ke; ++kk) fold_bin_add_generic<R, SHARE_P>(sp[kk], invP, cc, n_phi, rs, hb, sink);
 }
 
 // S4, first half: close magnitude bin `seg_i`.  fetch_word reads and clears this thread's counter word of phase bin j
@@ -137,20 +145,21 @@ __device__ __forceinline__ uint32_t fetch_word(const int j, const int n_phi, con
     return w;
 }
 
+// DUMP (gce_ce_debug_histogram): dpos[r] is the position of slot r's trial in the caller's list (-1: not listed); the
+// count this word contributes to Eq. 4 is written to out_counts[lc][dpos][j][seg_i].
 template <int R, bool DUMP, bool BIG>
 __device__ __forceinline__ void close_word(const uint32_t w, const int j, const int w2, const int n_phi, const uint32_t us,
                                            int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
-                                           const int lc, const int64_t s0, const bool (&valid)[R], const int seg_i) {
+                                           const int lc, const int (&dpos)[R], const int seg_i) {
     int64_t v0, v1;
     ltab_pair<BIG>(sL, prm.ltab, w, us, v0, v1);
     S2[2 * w2] += v0;
     if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
     if (DUMP) {
         const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
-        if (valid[2 * w2])
-            prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2) * n_phi + j) * prm.n_m + seg_i] = c0;
-        if (2 * w2 + 1 < R && valid[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0])
-            prm.out_counts[(((int64_t)lc * prm.n_trials + s0 + 2 * w2 + 1) * n_phi + j) * prm.n_m + seg_i] = c1;
+        const int d0 = dpos[2 * w2], d1 = dpos[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0];
+        if (d0 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d0) * n_phi + j) * prm.n_m + seg_i] = c0;
+        if (2 * w2 + 1 < R && d1 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d1) * n_phi + j) * prm.n_m + seg_i] = c1;
     }
 }
 
@@ -166,7 +175,7 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
                                               const uint32_t (&hb)[(R + 1) / 2],
                                               uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
                                               const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
-                                              const int64_t s0, const bool (&valid)[R], const int seg_i) {
+                                              const int (&dpos)[R], const int seg_i) {
     constexpr int RW = (R + 1) / 2;
     uint32_t prev[RW], first[RW];
     if (NPHI > 0) {
@@ -186,10 +195,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
                     const uint32_t ww = w[jj][w2];
                     if (REGM) mg[REGM ? j0 + jj : 0][w2] += ww;
                     else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, ww);
-                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                     else {
                         if (j0 + jj == 0) first[w2] = ww;
-                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                         prev[w2] = ww;
                     }
                 }
@@ -200,10 +209,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
             for (int w2 = 0; w2 < RW; ++w2) {
                 const uint32_t ww = fetch_word<EXT>(j, n_phi, rs, hb[w2]);
                 red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, ww);
-                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                 else {
                     if (j == 0) first[w2] = ww;
-                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                     prev[w2] = ww;
                 }
             }
@@ -212,23 +221,73 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
     if (OVL) {  // bin 0 = cells n_phi-1 and 0
 #pragma unroll
         for (int w2 = 0; w2 < RW; ++w2)
-            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, us, S2, sL, prm, lc, s0, valid, seg_i);
+            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
     }
 }
 
-// NPHI > 0: compile-time n_phi (unrolled S4); NPHI == 0: any n_phi <= 64.  REGM: phase marginal in registers, exactly
-// 512 threads per CTA; otherwise the marginal is a second set of counter rows in shared memory, threads per CTA =
-// prm.nt (any multiple of 32 up to 640), which leaves registers for a fifth warp per sub-partition when the shared
-// memory allows it.  R = trials per thread.  SHARE_P: the R trials of a thread share one period (n_pdot % R == 0).
-// DUMP: test mode, trials come from a list and the count tables are written out.
-template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT>
-__global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchParams prm) {
+// Per-trial constants of the R consecutive trial slots s0 .. s0 + R - 1 of one thread:
+// invP = 1/P, c = ((-0.5 * Pdot) * invP) * invP.  fast: every |y| of the light curve stays below 2^51, so the magic-add
+// floors are exact; pz: every c is +-0 (then x = a bit for bit).  Shared by k_search and k_debug_bins.
+template <int R, bool SHARE_P>
+__device__ __forceinline__ void trial_slot_constants(const SearchParams &prm, const int64_t s0, const double nphi_d,
+                                                     const double dt_max, double (&invP)[R], double (&cc)[R],
+                                                     int64_t (&qv)[R], bool (&valid)[R], bool &fast, bool &pz) {
+    fast = true;
+    pz = true;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t s = s0 + r;
+        valid[r] = s < prm.n_trials;
+        const int64_t q = valid[r] ? s : 0;
+        qv[r] = q + prm.q_off;  // reported index: flat q of the caller's whole grid
+        double ip = 0.0, c = 0.0;
+        if (valid[r] && (!SHARE_P || r == 0)) ip = __ddiv_rn(1.0, prm.periods[q / prm.n_pdot]);
+        if (SHARE_P && r > 0) ip = invP[0];
+        if (valid[r]) c = __dmul_rn(__dmul_rn(__dmul_rn(-0.5, prm.pdots[q % prm.n_pdot]), ip), ip);
+        invP[r] = ip;
+        cc[r] = c;
+        // conservative bound on |y|: below 2^51 the magic-add floors are exact
+        fast = fast && (nphi_d * (dt_max * fabs(ip) + dt_max * dt_max * fabs(c)) * 1.000001 < kYSafe);
+        pz = pz && (c == 0.0);
+    }
+}
+
+// EXT: sort the thread's trial slots by c, largest first (so x_0 >= x_1 >= ... for every point: dt2 >= 0 and RN is
+// monotone), keeping qv / valid / org with their trial, and report how far apart the phases get over the light curve:
+// pair_ok: the two trials of every counter word stay within one cycle, quad_ok: all R trials do.
+template <int R>
+__device__ __forceinline__ void sort_slots_by_c(double (&cc)[R], int64_t (&qv)[R], bool (&valid)[R], int (&org)[R],
+                                                const double dt_max, bool &pair_ok, bool &quad_ok) {
+    auto cswap = [&](const int i, const int j) {  // compare-exchange: afterwards cc[i] >= cc[j]
+        if (cc[i] < cc[j]) {
+            const double tc = cc[i]; cc[i] = cc[j]; cc[j] = tc;
+            const int64_t tq = qv[i]; qv[i] = qv[j]; qv[j] = tq;
+            const bool tv = valid[i]; valid[i] = valid[j]; valid[j] = tv;
+            const int to = org[i]; org[i] = org[j]; org[j] = to;
+        }
+    };
+    if (R == 4) { cswap(0, 1 % R); cswap(2 % R, 3 % R); cswap(0, 2 % R); cswap(1 % R, 3 % R); cswap(1 % R, 2 % R); }
+    else cswap(0, 1 % R);
+    const double d2 = dt_max * dt_max;
+#pragma unroll
+    for (int w2 = 0; w2 < (R + 1) / 2; ++w2) pair_ok = pair_ok && ((cc[2 * w2] - cc[(2 * w2 + 1) % R]) * d2 < 0.999);
+    quad_ok = quad_ok && ((cc[0] - cc[R - 1]) * d2 < 0.999);
+}
+
+// NPHI > 0: compile-time n_phi (unrolled S4); NPHI == 0: any n_phi <= 64.  REGM: phase marginal in registers (needs a
+// compile-time n_phi); otherwise the marginal is a second set of counter rows in shared memory.  NTC: compile-time
+// threads per CTA, or 0 = blockDim.x (any multiple of 32 up to 640).  R = trials per thread.  SHARE_P: the R trials of a
+// thread share one period (n_pdot % R == 0).  EXT: 2 n_phi + 1 counter rows, shared floors (fold_bin_add MODE 1 / 2).
+// DUMP (gce_ce_debug_histogram): the same kernel, plan and tiles as the search, but only tiles that hold a listed trial
+// are processed and, instead of the search outputs, the count tables (and CE) of the listed trials are written.
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT, int NTC>
+__global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchParams prm) {
     static_assert(!REGM || NPHI > 0, "register marginals need a compile-time n_phi");
-    static_assert(!EXT || (SHARE_P && !DUMP && R % 2 == 0), "extended rows serve trial pairs that share a period");
+    static_assert(!EXT || (SHARE_P && R % 2 == 0), "extended rows serve trial pairs that share a period");
     constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
     constexpr int NPHI_REG = REGM ? NPHI : 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int NT = REGM ? 512 : (int)blockDim.x, NW = NT >> 5;
+    const int NT = NTC > 0 ? NTC : (int)blockDim.x, NW = NT >> 5;
     const int tid = threadIdx.x, lane = tid & 31;
     const int n_phi = NPHI > 0 ? NPHI : prm.n_phi, n_m = prm.n_m;
     const uint32_t rs = (uint32_t)NT * 4u;  // bytes between the counter rows of consecutive phase bins
@@ -293,10 +352,10 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     uint32_t hb[RW];
 #pragma unroll
     for (int w2 = 0; w2 < RW; ++w2) hb[w2] = smem_u32(hist) + (uint32_t)tid * 4u + (uint32_t)w2 * plane;
-    const bool ovl = !DUMP && prm.overlap != 0;  // N2: 2N table entries per trial
+    const bool ovl = prm.overlap != 0;  // N2: 2N table entries per trial
     const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)(ovl ? 2 * N : N) : 0.0;
     const uint32_t us = ((ovl ? 2 : 1) * N <= 8191) ? 3u : 0u;  // counter unit 2^us: a field is its table entry's byte offset
-    const uint32_t inc0 = 1u << us, inc1 = 0x10000u << us;
+    const RedSink sink{1u << us, 0x10000u << us};
     uint32_t mg[NPHI_REG][RW];  // phase marginal n_j of the R trials (NPHI > 0), packed like the histogram
 #pragma unroll
     for (int j = 0; j < NPHI_REG; ++j)
@@ -315,53 +374,42 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     int g = 0;  // position in this CTA's chunk sequence (streamed mode)
     for (int tl = 0; tl < n_tiles; ++tl) {
         const int64_t s0 = (tile_lo + tl) * TILE + (int64_t)tid * R;  // first trial slot of this thread
+        if (DUMP && single) {  // skip tiles without a listed trial (streamed tiles keep their place in the chunk sequence)
+            bool any = false;
+            const int64_t t0q = (tile_lo + tl) * TILE;
+            for (int64_t i = tid; i < prm.n_dump; i += NT) {
+                const int64_t q = prm.trial_q[i];
+                any = any || (q >= t0q && q < t0q + TILE);
+            }
+            if (!__syncthreads_or(any)) continue;
+        }
         // ---- per-trial constants
         double invP[R], cc[R];  // SHARE_P: only invP[0] is used
         int64_t qv[R];
         bool valid[R];
-        bool fast = true, pz = true;
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int64_t s = s0 + r;
-            valid[r] = s < prm.n_trials;
-            int64_t q = 0;
-            if (valid[r]) q = DUMP ? prm.trial_q[s] : s;
-            qv[r] = q + prm.q_off;  // reported index: flat q of the caller's whole grid
-            double ip = 0.0, c = 0.0;
-            if (valid[r] && (!SHARE_P || r == 0)) ip = __ddiv_rn(1.0, prm.periods[q / prm.n_pdot]);
-            if (SHARE_P && r > 0) ip = invP[0];
-            if (valid[r]) c = __dmul_rn(__dmul_rn(__dmul_rn(-0.5, prm.pdots[q % prm.n_pdot]), ip), ip);
-            invP[r] = ip;
-            cc[r] = c;
-            // conservative bound on |y|: below 2^51 the magic-add floors are exact
-            fast = fast && (nphi_d * (dt_max * fabs(ip) + dt_max * dt_max * fabs(c)) * 1.000001 < kYSafe);
-            pz = pz && (c == 0.0);
-        }
+        bool fast, pz;
+        trial_slot_constants<R, SHARE_P>(prm, s0, nphi_d, dt_max, invP, cc, qv, valid, fast, pz);
         fast = __all_sync(0xffffffffu, fast);
         pz = __all_sync(0xffffffffu, pz);
-        // EXT: sort the thread's trials by c, largest first (so x_0 >= x_1 >= ... for every point: dt2 >= 0 and RN is
-        // monotone), remember which trial sits in which slot, and check how far apart the phases get over the light curve
         int org[R];  // trial (0..R-1, relative to s0) held by slot r
 #pragma unroll
         for (int r = 0; r < R; ++r) org[r] = r;
         bool pair_ok = EXT && fast && !pz, quad_ok = pair_ok;
         if (EXT) {
-            auto cswap = [&](const int i, const int j) {  // compare-exchange: afterwards cc[i] >= cc[j]
-                if (cc[i] < cc[j]) {
-                    const double tc = cc[i]; cc[i] = cc[j]; cc[j] = tc;
-                    const int64_t tq = qv[i]; qv[i] = qv[j]; qv[j] = tq;
-                    const bool tv = valid[i]; valid[i] = valid[j]; valid[j] = tv;
-                    const int to = org[i]; org[i] = org[j]; org[j] = to;
-                }
-            };
-            if (R == 4) { cswap(0, 1 % R); cswap(2 % R, 3 % R); cswap(0, 2 % R); cswap(1 % R, 3 % R); cswap(1 % R, 2 % R); }
-            else cswap(0, 1 % R);
-            const double d2 = dt_max * dt_max;
-#pragma unroll
-            for (int w2 = 0; w2 < RW; ++w2) pair_ok = pair_ok && ((cc[2 * w2] - cc[(2 * w2 + 1) % R]) * d2 < 0.999);
-            quad_ok = quad_ok && ((cc[0] - cc[R - 1]) * d2 < 0.999);
+            sort_slots_by_c<R>(cc, qv, valid, org, dt_max, pair_ok, quad_ok);
             pair_ok = __all_sync(0xffffffffu, pair_ok);
             quad_ok = __all_sync(0xffffffffu, quad_ok);
+        }
+        int dpos[R];  // DUMP: position of the slot's trial in the caller's list
+#pragma unroll
+        for (int r = 0; r < R; ++r) dpos[r] = -1;
+        if (DUMP) {
+            for (int64_t i = 0; i < prm.n_dump; ++i) {
+                const int64_t q = prm.trial_q[i];
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    if (valid[r] && qv[r] == q) dpos[r] = (int)i;
+            }
         }
 
         int64_t S2[R];
@@ -371,7 +419,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
         int seg_s = 0;  // magnitude bins finished so far, counted in this warp's (rotated) order
         for (int c = 0; c < n_chunks; ++c) {
             const int buf = single ? 0 : (g & 1);
-            if (!single || tl == 0) mbar_wait(&full[buf], single ? 0u : (uint32_t)((g >> 1) & 1));
+            if (!single || tl == 0 || DUMP) mbar_wait(&full[buf], single ? 0u : (uint32_t)((g >> 1) & 1));
             const double2 *sp = spts + (size_t)buf * CH;
             const int k_base = c * CH;
             const int k_end = min(N, k_base + CH);
@@ -383,12 +431,12 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-                        if (pz) fold_range<R, SHARE_P, true, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-                        else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
-                        else fold_range<R, SHARE_P, false, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, inc0, inc1);
+                        if (pz) fold_range<R, SHARE_P, true, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        else fold_range<R, SHARE_P, false, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
                     } else {
-                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, inc0, inc1);
+                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, sink);
                     }
                 }
                 if (b1 > k_end) break;  // the bin continues in the next buffer
@@ -397,14 +445,14 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                     // a cell of this bin holds at most b1 - b0 points (twice that with overlapping bins)
                     if (!ovl) {
                         if (us == 3u && b1 - b0 < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, DUMP, false, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, DUMP, true, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
-                    } else if (!DUMP) {
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                    } else {
                         if (us == 3u && 2 * (b1 - b0) < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, false, false, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, false, true, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, s0, valid, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                     }
                 }
                 ++seg_s;
@@ -467,10 +515,10 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
         if (DUMP) {
 #pragma unroll
             for (int r = 0; r < R; ++r)
-                if (valid[r] && prm.out_ce_at) prm.out_ce_at[(int64_t)lc * prm.n_trials + s0 + r] = ce[r];
+                if (dpos[r] >= 0 && prm.out_ce_at) prm.out_ce_at[(int64_t)lc * prm.n_dump + dpos[r]] = ce[r];
         } else {
             if (prm.out_ce) {
-                const int64_t o = (int64_t)lc * prm.n_trials + s0;  // q == slot outside DUMP
+                const int64_t o = (int64_t)lc * prm.n_trials + s0;
                 float *o32 = reinterpret_cast<float *>(prm.out_ce) + o;
                 double cet[R];  // CE in trial order (EXT has sorted the slots by c)
 #pragma unroll
@@ -505,7 +553,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     if (!valid[r]) continue;
-                    const int64_t d = S[r] - K;   // |d| < 2^60
+                    const int64_t d = S[r] - K;   // |d| <= max(S, K) < 2^61
                     a += d;
                     b += (u128_t)((__int128)d * d);
                     mn = S[r] < mn ? S[r] : mn;
@@ -515,7 +563,7 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
                 u128_t au = (u128_t)a;
                 for (int o = 16; o > 0; o >>= 1) {
                     au += shfl_xor_u128(au, o);
-                    b += shfl_xor_u128(b, o);            // <= 32 * R * 2^120 < 2^128
+                    b += shfl_xor_u128(b, o);            // <= 32 * R * 2^122 < 2^128
                     const int64_t m2 = __shfl_xor_sync(0xffffffffu, mn, o), m3 = __shfl_xor_sync(0xffffffffu, mx, o);
                     mn = m2 < mn ? m2 : mn;
                     mx = m3 > mx ? m3 : mx;
@@ -565,5 +613,28 @@ __global__ void __launch_bounds__(REGM ? 512 : 640, 1) k_search(const SearchPara
     }
 }
 
+// Host side of one instantiation: opt in to the dynamic shared memory once per device, then launch.
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT, int NTC>
+cudaError_t launch_search(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
+    auto kern = k_search<NPHI, REGM, R, SHARE_P, DUMP, EXT, NTC>;
+    static std::mutex mu;
+    static size_t smem_set[64] = {};  // largest opt-in made so far, per device
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (plan.smem > smem_set[dev]) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem);
+            if (e != cudaSuccess) return e;
+            smem_set[dev] = plan.smem;
+        }
+    }
+    if (NTC > 0 && plan.nt != NTC) return cudaErrorInvalidValue;
+    const unsigned grid = (unsigned)((int64_t)n_lc * plan.jobs_per_lc);
+    kern<<<grid, plan.nt, plan.smem, st>>>(sp);
+    return cudaGetLastError();
+}
 
 }  // namespace

@@ -78,9 +78,10 @@ __global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__
     const double mean_d = sum_d / n;
     double var = sum_d2 / n - mean_d * mean_d;
     if (var < 0.0 || acc[6] == acc[7]) var = 0.0;  // min == max: every trial has the same CE, the spread is exactly 0
+    const double mn = (double)(int64_t)acc[6] * scale;
+    if (acc[6] == acc[7]) { o[0] = mn; o[1] = 0.0; o[2] = mn; o[3] = CUDART_NAN; return; }  // one CE value only: mean = min exactly
     const double mean = ((double)pivot + mean_d) * scale;
     const double sd = sqrt(var) * scale;
-    const double mn = (double)(int64_t)acc[6] * scale;
     o[0] = mean; o[1] = sd; o[2] = mn; o[3] = (mean - mn) / sd;
 }
 

@@ -55,8 +55,12 @@ def test_workspace_and_error_codes_on_host(gce):
         assert e.value.code == -2
     with pytest.raises(gce.GceError):
         gce.gce_ce_workspace_bytes(-1, 1, 10, 1, prm)
-    assert gce.gce_ce_launch_count(3, prm) == 4
-    assert gce.gce_ce_launch_count(3, gce.make_params(20, 10)) == 3
+    # preprocess (+ table), search, merge_topk; + merge_stats with Eq. 5 statistics or a partial blob
+    assert gce.gce_ce_launch_count(3, 100, prm) == 3
+    assert gce.gce_ce_launch_count(3, 100, gce.make_params(20, 10)) == 2
+    assert gce.gce_ce_launch_count(3, 100, prm, partial=True) == 4
+    assert gce.gce_ce_launch_count(3, 0, gce.make_params(20, 10, top_k=1, want_stats=True)) == 3
+    assert gce.gce_ce_launch_count(0, 100, prm) == 0
 
 
 def test_validate_host(gce):

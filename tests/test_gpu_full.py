@@ -11,7 +11,8 @@ import pytest
 import torch
 
 import gce_workloads as W
-from test_gpu_parity import RTOL32, RTOL64, assert_ce_close, assert_topk_matches, dev, run_search
+from test_gpu_parity import (RTOL32, RTOL64, assert_ce_close, assert_counts_match_oracle, assert_topk_matches, dev,
+                             run_search)
 
 pytestmark = pytest.mark.gpu
 
@@ -120,6 +121,82 @@ def test_c5_full_top16(gce, oracle):
         kth = ce_nb[np.searchsorted(nb, gi[-1])]
         better = nb[ce_nb < kth * (1 - RTOL64) - 1e-13]
         assert set(better.tolist()) <= set(gi.tolist())
+
+
+# ------------------------------------------------------------------------------------------ counts of the timed kernels
+def _fold_modes_of(gce, w, lc, qs):
+    """Fold variant the owning thread of each trial qualifies for (gce_ce_debug_bins, FOLD_AUTO)."""
+    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins)
+    t, m, o, p, pd = dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots)
+    n = int(w.lc_offsets[lc + 1] - w.lc_offsets[lc])
+    pb = torch.empty(n, dtype=torch.int32, device="cuda")
+    mb = torch.empty(n, dtype=torch.int32, device="cuda")
+    mode = torch.empty(1, dtype=torch.int32, device="cuda")
+    out = []
+    for q in qs:
+        gce.gce_ce_debug_bins(t, m, o, p, pd, prm, lc, int(q), pb, mb, out_fold_mode=mode)
+        out.append(int(mode.item()))
+    return out
+
+
+def _tile_edge_trials(n_trials, tile, rng, n_random):
+    """First / last trial, both sides of the first tile boundaries and of a boundary deep in the grid, plus a random sample."""
+    deep = (n_trials // tile // 2) * tile
+    edge = [0, 1, 3, 4, tile - 1, tile, tile + 1, 2 * tile - 1, 2 * tile, deep - 1, deep, deep + 5, n_trials - 2, n_trials - 1]
+    q = np.concatenate([np.array(edge), rng.integers(0, n_trials, size=n_random)])
+    return np.unique(q[(q >= 0) & (q < n_trials)]).astype(np.int64)
+
+
+def test_c3_full_counts_of_the_timed_kernel(gce, oracle):
+    """configs[2] at full size: the kernel bench.py times (n_phi = 20, 4 trials per thread sharing a period, shared floors,
+    512 threads: k_search<20,1,4,1,.,1,512>) in dump mode -- histogram counts bit-exact against the oracle on all 64 light
+    curves, at tile edges, and in both the quad (long periods) and the pair (short periods) shared-floor variants."""
+    w = W.make("C3")
+    n_pd = w.pdots.size
+    n_trials = w.periods.size * n_pd
+    rng = np.random.default_rng(303)
+    short_p = (w.periods.size - 1 - rng.integers(0, 2000, size=6)) * n_pd + rng.integers(0, n_pd, size=6)  # P ~ 120 s
+    q = np.unique(np.concatenate([_tile_edge_trials(n_trials, 2048, rng, 24), short_p]))
+    modes = set(_fold_modes_of(gce, w, 0, q))
+    assert {gce.binding.FOLD_QUAD, gce.binding.FOLD_PAIR} <= modes, modes
+    assert_counts_match_oracle(gce, oracle, w, q)
+
+
+def test_c5_full_counts_of_the_timed_kernel(gce, oracle):
+    """configs[4] at full size: k_search<30,1,4,1,.,0,512> in dump mode, all 16 light curves of 5000 points (magnitude bins
+    above 1024 points: the table's global tail), counts bit-exact at tile edges and on a random sample."""
+    w = W.make("C5")
+    n_trials = w.periods.size * w.pdots.size
+    rng = np.random.default_rng(505)
+    q = _tile_edge_trials(n_trials, 2048, rng, 20)
+    assert_counts_match_oracle(gce, oracle, w, q)
+
+
+def test_c4_full_counts_of_the_timed_kernel(gce, oracle):
+    """configs[3] at full size: k_search<15,1,4,0,.,0,512> (Pdot = {0}: the 4 trials of a thread are 4 periods) in dump
+    mode, bit-exact counts on a sample of the 1000 light curves (the dump runs all of them)."""
+    w = W.make("C4")
+    rng = np.random.default_rng(404)
+    q = _tile_edge_trials(w.periods.size, 2048, rng, 20)
+    assert_counts_match_oracle(gce, oracle, w, q, lcs=[0, 1, 2, 250, 499, 777, 998, 999])
+
+
+def test_c2_full_counts_of_the_timed_kernel(gce, oracle):
+    w = W.make("C2")
+    rng = np.random.default_rng(202)
+    q = _tile_edge_trials(w.periods.size, 2048, rng, 20)
+    assert_counts_match_oracle(gce, oracle, w, q, lcs=[0, 1, 50, 98, 99])
+
+
+def test_paper_binning_counts_of_the_timed_kernel(gce, oracle):
+    """The paper's production binning (50 overlapping phase bins x 10) on the C3 grid: k_search<50,1,2,1,.,0,512>
+    in dump mode writes the overlapped table; bit-exact against oracle.overlap_counts(oracle.histogram)."""
+    w = W.make("C3", n_lc=8)
+    w.n_phase_bins, w.n_mag_bins = 50, 10
+    rng = np.random.default_rng(5050)
+    q = _tile_edge_trials(w.periods.size * w.pdots.size, 1024, rng, 16)
+    assert_counts_match_oracle(gce, oracle, w, q, overlap=True)
+    assert_counts_match_oracle(gce, oracle, w, q[:8], overlap=False)
 
 
 def test_c5_cube_mode_sampled(gce, oracle):

@@ -75,72 +75,166 @@ def assert_topk_matches(ref_row, gpu_idx, gpu_val, k, rtol, oracle):
 
 
 # ------------------------------------------------------------------------------------------ bins (S1, S2)
-@pytest.mark.parametrize("n_phi,n_m", [(20, 10), (15, 8), (30, 10), (50, 10), (1, 1), (64, 64), (7, 3)])
-def test_debug_bins_bit_exact(gce, oracle, n_phi, n_m):
-    w = W.random_batch(100 + n_phi, n_lc=3, n_min=1, n_max=700, n_p=40, n_pdot=5, n_phase_bins=n_phi,
-                       n_mag_bins=n_m, pdot_range=(-2e-9, 3e-10))
+def _debug_bins_all_modes(gce, oracle, w, lcs, qs, expect_modes=None):
+    """gce_ce_debug_bins (the search kernel's own fold functions) against oracle.fold_bins for every fold variant whose
+    precondition holds for the trial: all of them must give the oracle's bins.  Returns the set of variants seen."""
+    n_phi, n_m, n_pdot = w.n_phase_bins, w.n_mag_bins, w.pdots.size
     prm = gce.make_params(n_phi, n_m)
     t, m, o, p, pd = dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots)
-    for lc in range(w.n_lc):
+    mode_gpu = torch.empty(1, dtype=torch.int32, device="cuda")
+    seen = set()
+    for lc in lcs:
         a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
         dt, dt2, mbin = oracle.preprocess(w.times[a:b], w.mags[a:b], n_m)
         pb_gpu = torch.empty(b - a, dtype=torch.int32, device="cuda")
         mb_gpu = torch.empty(b - a, dtype=torch.int32, device="cuda")
-        for q in (0, 7, 93, 199):
-            gce.gce_ce_debug_bins(t, m, o, p, pd, prm, lc, q, pb_gpu, mb_gpu)
-            pb, _ = oracle.fold_bins(dt, dt2, w.periods[q // 5], w.pdots[q % 5], n_phi)
-            assert np.array_equal(pb_gpu.cpu().numpy(), pb)
-            assert np.array_equal(mb_gpu.cpu().numpy(), mbin)
+        for q in qs:
+            pb, _ = oracle.fold_bins(dt, dt2, w.periods[q // n_pdot], w.pdots[q % n_pdot], n_phi)
+            for mode in (gce.binding.FOLD_AUTO, gce.binding.FOLD_PLAIN, gce.binding.FOLD_PAIR, gce.binding.FOLD_QUAD,
+                         gce.binding.FOLD_GENERIC, gce.binding.FOLD_PDOT_ZERO):
+                gce.gce_ce_debug_bins(t, m, o, p, pd, prm, lc, q, pb_gpu, mb_gpu, fold_mode=mode, out_fold_mode=mode_gpu)
+                used = int(mode_gpu.item())
+                if used < 0:       # this variant's precondition does not hold for the trial
+                    assert mode != gce.binding.FOLD_AUTO and mode != gce.binding.FOLD_GENERIC
+                    assert bool(torch.all(pb_gpu == -1)) or b == a
+                    continue
+                assert mode == gce.binding.FOLD_AUTO or used == mode
+                seen.add(used)
+                assert np.array_equal(pb_gpu.cpu().numpy(), pb), (lc, q, mode, used)
+                assert np.array_equal(mb_gpu.cpu().numpy(), mbin)
+    if expect_modes is not None:
+        assert expect_modes <= seen, (expect_modes, seen)
+    return seen
+
+
+@pytest.mark.parametrize("n_phi,n_m", [(20, 10), (15, 8), (30, 10), (50, 10), (1, 1), (64, 64), (7, 3)])
+def test_debug_bins_bit_exact(gce, oracle, n_phi, n_m):
+    """Pdot of both signs, 5 Pdots per period (odd: the 4 trials of a thread straddle periods, or R = 2 for n_phi = 50)."""
+    w = W.random_batch(100 + n_phi, n_lc=3, n_min=1, n_max=700, n_p=40, n_pdot=5, n_phase_bins=n_phi,
+                       n_mag_bins=n_m, pdot_range=(-2e-9, 3e-10))
+    _debug_bins_all_modes(gce, oracle, w, range(w.n_lc), (0, 7, 93, 199))
+
+
+@pytest.mark.parametrize("n_phi,n_pdot", [(20, 8), (30, 4), (15, 64), (50, 2), (64, 4)])
+def test_debug_bins_shared_floor_variants(gce, oracle, n_phi, n_pdot):
+    """Grids whose Pdot values share a period inside a thread: the pair / quad shared-floor variants (fold_bin_add MODE 1 /
+    2) and the fold-back of the extended rows must reproduce the oracle's bins, also where they only just qualify."""
+    w = W.make("C3", n_lc=2, n_p=60, n_pdot=n_pdot)
+    w.n_phase_bins = n_phi
+    qs = [0, 1, n_pdot - 1, 17 * n_pdot + 2, 59 * n_pdot + n_pdot - 1]
+    expect = {gce.binding.FOLD_PLAIN, gce.binding.FOLD_GENERIC, gce.binding.FOLD_PAIR}
+    if n_phi != 50:
+        expect.add(gce.binding.FOLD_QUAD)   # R = 4 trials per thread
+    seen = _debug_bins_all_modes(gce, oracle, w, range(w.n_lc), qs, expect)
+    # a trial with Pdot = 0 exactly next to non-zero ones is not a PDOT_ZERO thread
+    assert gce.binding.FOLD_PDOT_ZERO not in seen
+    # wide Pdot spacing: the trials of a thread drift apart by more than a cycle -> no shared floor
+    w2 = W.make("C5", n_lc=1, n_p=40, n_pdot=n_pdot)
+    w2.n_phase_bins = n_phi
+    _debug_bins_all_modes(gce, oracle, w2, [0], [0, 3 * n_pdot + 1, 39 * n_pdot + n_pdot - 1])
+
+
+def test_debug_bins_pdot_zero_grid(gce, oracle):
+    w = W.make("C4", n_lc=2, n_p=50)
+    seen = _debug_bins_all_modes(gce, oracle, w, range(2), (0, 13, 49))
+    assert gce.binding.FOLD_PDOT_ZERO in seen
+
+
+def _huge_cycle_workloads(n_phi, n_pdot=4):
+    """Two grids on a 3e9 s baseline.  A: Pdot up to +2e-7 makes x negative (floored modulus, reading Q5) and |y| exceeds
+    2^32 but not 2^51 (magic-add floors).  B: P ~ 1e-5 s puts |y| beyond 2^51 (the 64-bit generic fold; |y| < 2^62)."""
+    rng = np.random.default_rng(3)
+    t = np.sort(rng.uniform(0, 3.0e9, size=400))
+    m = rng.normal(size=400)
+    offs = np.array([0, 250, 400], dtype=np.int64)
+    pd_a = np.array([-1e-9, 0.0, 5e-8, 2e-7, 1e-8, -3e-8, 7e-8, 1e-7])[:n_pdot]
+    pd_b = np.array([-1e-13, 0.0, 2e-13, 1e-13, 3e-13, -2e-13, 5e-14, 4e-13])[:n_pdot]
+    wa = W.Workload("hugeA", t, m, offs, np.array([0.37, 1.0, 55.0, 420.0]), pd_a, n_phi, 10, 1, True)
+    wb = W.Workload("hugeB", t, m, offs, np.array([1e-5, 2.5e-5, 1.7e-5]), pd_b, n_phi, 10, 1, True)
+    return wa, wb
+
+
+def _y_range(oracle, w, lc=0):
+    a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
+    dt, dt2, _ = oracle.preprocess(w.times[a:b], w.mags[a:b], w.n_mag_bins)
+    x_min, y_abs = 0.0, []
+    for P in w.periods:
+        for Pd in w.pdots:
+            _, x = oracle.fold_bins(dt, dt2, P, Pd, w.n_phase_bins)
+            x_min = min(x_min, x.min())
+            y_abs.append(w.n_phase_bins * np.abs(x).max())
+    return x_min, np.array(y_abs)
 
 
 def test_debug_bins_huge_cycle_counts_take_the_slow_path(gce, oracle):
-    """|n_phi * x| beyond the 32-bit fast range (and negative x for Pdot > 0) must still be bit-exact."""
-    rng = np.random.default_rng(3)
-    t = np.sort(rng.uniform(0, 3.0e9, size=300))
-    m = rng.normal(size=300)
-    periods = np.array([0.37, 1.0, 55.0, 420.0])
-    pdots = np.array([-1e-9, 0.0, 5e-8])
-    prm = gce.make_params(50, 10)
-    dt, dt2, mbin = oracle.preprocess(t, m, 10)
-    args = [dev(t), dev(m), dev(np.array([0, 300])), dev(periods), dev(pdots)]
-    pb_gpu = torch.empty(300, dtype=torch.int32, device="cuda")
-    mb_gpu = torch.empty(300, dtype=torch.int32, device="cuda")
-    x_min, y_max = 0.0, 0.0
-    for q in range(12):
-        gce.gce_ce_debug_bins(*args, prm, 0, q, pb_gpu, mb_gpu)
-        pb, x = oracle.fold_bins(dt, dt2, periods[q // 3], pdots[q % 3], 50)
-        assert np.array_equal(pb_gpu.cpu().numpy(), pb), q
-        x_min, y_max = min(x_min, x.min()), max(y_max, 50 * np.abs(x).max())
-    assert x_min < 0          # a Pdot > 0 trial really went negative (floored modulus, reading Q5)
-    assert y_max > 2.0 ** 32  # and a trial really left the 32-bit fast range
+    """Negative x, |y| beyond 2^32 and beyond 2^51: bit-exact in every fold variant that qualifies."""
+    wa, wb = _huge_cycle_workloads(50)
+    x_min, y = _y_range(oracle, wa)
+    assert x_min < 0 and np.any(y > 2.0 ** 32) and np.all(y < 2.0 ** 51)
+    seen = _debug_bins_all_modes(gce, oracle, wa, [0, 1], range(wa.periods.size * wa.pdots.size))
+    assert gce.binding.FOLD_PLAIN in seen
+    _, y = _y_range(oracle, wb)
+    assert np.all(y > 2.0 ** 51) and np.all(y < 2.0 ** 62)
+    seen = _debug_bins_all_modes(gce, oracle, wb, [0, 1], range(wb.periods.size * wb.pdots.size))
+    assert seen == {gce.binding.FOLD_GENERIC}      # nothing else qualifies
 
 
 # ------------------------------------------------------------------------------------------ counts (S3)
+def dump_counts(gce, w, q, overlap=False, want_ce=True):
+    """gce_ce_debug_histogram: the search kernel of w's grid in dump mode -> (counts [n_lc][len(q)][n_phi][n_m], ce)."""
+    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins, overlap=overlap)
+    ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, w.periods.size, w.pdots.size, prm),
+                     dtype=torch.uint8, device="cuda")
+    counts = torch.empty((w.n_lc, len(q), w.n_phase_bins, w.n_mag_bins), dtype=torch.int32, device="cuda")
+    ce_at = torch.empty((w.n_lc, len(q)), dtype=torch.float64, device="cuda") if want_ce else None
+    gce.gce_ce_debug_histogram(dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots), prm,
+                               dev(np.asarray(q, dtype=np.int64)), counts, ce_at, ws)
+    torch.cuda.synchronize()
+    return counts.cpu().numpy().astype(np.int64), (ce_at.cpu().numpy() if want_ce else None)
+
+
+def assert_counts_match_oracle(gce, oracle, w, q, overlap=False, lcs=None):
+    counts, ce = dump_counts(gce, w, q, overlap)
+    q = np.asarray(q, dtype=np.int64)
+    for lc in (range(w.n_lc) if lcs is None else lcs):
+        a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
+        ref = oracle.histogram(w.times[a:b], w.mags[a:b], w.periods, w.pdots, w.n_phase_bins, w.n_mag_bins, q)
+        if overlap:
+            ref = np.stack([oracle.overlap_counts(r) for r in ref]) if len(q) else ref
+        assert np.array_equal(counts[lc], ref), (lc, np.argwhere(counts[lc] != ref)[:5])
+        assert np.all(counts[lc].sum(axis=(1, 2)) == (2 if overlap else 1) * (b - a))
+    ce_ref = oracle.ce_at(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, w.n_phase_bins, w.n_mag_bins, q, overlap=overlap)
+    sel = list(range(w.n_lc) if lcs is None else lcs)
+    assert_ce_close(ce[sel], ce_ref[sel], RTOL64)
+
+
 @pytest.mark.parametrize("seed,n_phi,n_m,n_p,n_pdot", [(1, 20, 10, 37, 4), (2, 15, 8, 300, 1), (3, 30, 10, 64, 7),
-                                                        (4, 50, 10, 5, 3), (5, 1, 4, 9, 2), (6, 64, 64, 33, 2)])
+                                                        (4, 50, 10, 5, 3), (5, 1, 4, 9, 2), (6, 64, 64, 33, 2),
+                                                        (7, 20, 10, 700, 8), (8, 15, 8, 90, 64), (9, 50, 10, 400, 2)])
 def test_histogram_counts_bit_exact(gce, oracle, seed, n_phi, n_m, n_p, n_pdot):
-    """Production search kernel in dump mode: counts identical to the oracle's for every sampled trial, on
-    ragged batches (incl. empty and 1-point light curves) longer than one shared-memory stage (512 points)."""
+    """The search kernel of the grid in dump mode (same plan, instantiation and tiles as gce_ce_search): counts identical
+    to the oracle's for every sampled trial, on ragged batches (incl. empty and 1-point light curves)."""
     w = W.random_batch(seed, n_lc=5, n_min=0, n_max=1500, n_p=n_p, n_pdot=n_pdot, n_phase_bins=n_phi, n_mag_bins=n_m)
     rng = np.random.default_rng(seed)
     T = n_p * n_pdot
     q = np.unique(np.concatenate([[0, T - 1], rng.integers(0, T, size=min(T, 70))])).astype(np.int64)
     rng.shuffle(q)
-    prm = gce.make_params(n_phi, n_m)
-    ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, q.size, 1, prm), dtype=torch.uint8, device="cuda")
-    counts = torch.empty((w.n_lc, q.size, n_phi, n_m), dtype=torch.int32, device="cuda")
-    ce_at = torch.empty((w.n_lc, q.size), dtype=torch.float64, device="cuda")
-    gce.gce_ce_debug_histogram(dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots), prm,
-                               dev(q), counts, ce_at, ws)
-    torch.cuda.synchronize()
-    counts = counts.cpu().numpy()
-    ce_ref = oracle.ce_at(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, n_phi, n_m, q)
-    for lc in range(w.n_lc):
-        a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
-        ref = oracle.histogram(w.times[a:b], w.mags[a:b], w.periods, w.pdots, n_phi, n_m, q)
-        assert np.array_equal(counts[lc].astype(np.int64), ref), lc
-        assert np.all(counts[lc].sum(axis=(1, 2)) == b - a)
-    assert_ce_close(ce_at.cpu().numpy(), ce_ref, RTOL64)
+    assert_counts_match_oracle(gce, oracle, w, q)
+    if seed in (1, 4, 7):
+        assert_counts_match_oracle(gce, oracle, w, q, overlap=True)
+
+
+@pytest.mark.parametrize("n_phi,n_pdot", [(20, 4), (30, 2), (15, 3), (50, 2), (64, 8)])
+def test_histogram_counts_huge_cycle_counts_through_the_search_kernel(gce, oracle, n_phi, n_pdot):
+    """The same two regimes through k_search itself (dump mode and the fp64 cube): negative x and |y| in (2^32, 2^51) on
+    the magic-add floors, |y| >= 2^51 on fold_range_generic -- for the shared-period R = 4 (n_pdot 4, 8), R = 2
+    (n_pdot 2) and period-straddling (n_pdot 3) kernels, extended-row and plain instantiations."""
+    for w in _huge_cycle_workloads(n_phi, n_pdot):
+        q = np.arange(w.periods.size * w.pdots.size)
+        assert_counts_match_oracle(gce, oracle, w, q)
+        ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, n_phi, 10)
+        res = run_search(gce, w, top_k=1, ce_fp64=True)
+        assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
 
 
 # ------------------------------------------------------------------------------------------ CE cube (S4) + selection (S5)
