@@ -38,11 +38,11 @@ thread_local int g_last_cuda_error = 0;
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-marginal kernels (<= 102 registers)
-constexpr int kMinPoints = 640;           // smallest point buffer; also the top-k merge scratch (16 B x 20 warps x 32)
+constexpr int kMinPoints = 640;           // smallest point buffer
 
-size_t search_smem_fixed() {
-    return sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) +
-           sizeof(uint64_t) * kMaxWarps * kStatWords;
+size_t search_smem_fixed() {  // mbarriers, seg row, Eq. 5 accumulators, the warps' top-k lists + thresholds, light-curve scalars
+    return sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) + sizeof(uint64_t) * kMaxWarps * kStatWords +
+           sizeof(int64_t) * kMaxWarps * 64 + sizeof(int64_t) * kMaxWarps * 2 + sizeof(double) * 2;
 }
 // counter rows of one thread: histogram (n_phi + 1 rows, the last one catches RN(x * n_phi) == n_phi * (floor(x) + 1)),
 // plus n_phi marginal rows when the marginal is not in registers; RW words each

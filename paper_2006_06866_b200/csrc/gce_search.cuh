@@ -117,6 +117,22 @@ __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int k
     for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE>(sp[kk], invP, cc, nphi_d, negn, rs, hb, sink);
 }
 
+#ifdef GCE_NOINLINE_FOLD
+// Experiment: the hot loop as a real call, so that the caller's cold state (phase marginals, top-k, tile bookkeeping) is
+// saved around it by the ABI instead of starving the loop of registers.  R = 4 trials sharing a period only.
+template <bool PZ, int MODE, int NPHI>
+__device__ __noinline__ void fold_range_call4(const double2 *__restrict__ sp, int kk, const int ke, const double invP0,
+                                              const double c0, const double c1, const double c2, const double c3,
+                                              const uint32_t rs, const uint32_t hb0, const uint32_t hb1,
+                                              const uint32_t inc0, const uint32_t inc1) {
+    const double invP[4] = {invP0, invP0, invP0, invP0};
+    const double cc[4] = {c0, c1, c2, c3};
+    const uint32_t hb[2] = {hb0, hb1};
+    const RedSink sink{inc0, inc1};
+    fold_range<4, true, PZ, MODE>(sp, kk, ke, invP, cc, (double)NPHI, 0u - (uint32_t)NPHI, rs, hb, sink);
+}
+#endif
+
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
 template <int R, bool SHARE_P, typename SINK>
 __device__ __forceinline__ void fold_bin_add_generic(const double2 p, const double (&invP)[R], const double (&cc)[R],
@@ -297,7 +313,13 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);                     // [2]
     int *sseg = reinterpret_cast<int *>(full + 2);                               // [n_m + 1] (<= 65)
     uint64_t *sstat = reinterpret_cast<uint64_t *>(sseg + GCE_CE_MAX_BINS + 4);  // [kMaxWarps][kStatWords]
-    uint32_t *hist = reinterpret_cast<uint32_t *>(sstat + kMaxWarps * kStatWords); // [RW][n_phi + 1][NT], 16-byte aligned
+    // Cold per-tile state lives in shared memory, not in registers, so that the hot loop has the register file to
+    // itself (it is register-starved: with the phase marginals in registers ptxas otherwise issues the dependent FP64
+    // instructions of a chain back to back): the warps' running top-k lists and the light curve's scalars.
+    int64_t *stop = reinterpret_cast<int64_t *>(sstat + kMaxWarps * kStatWords);  // [kMaxWarps][32] x (S, q), lane-sorted list
+    int64_t *sthr = stop + kMaxWarps * 64;                                       // [kMaxWarps] x (S, q) of the k-th element
+    volatile double *sinfo = reinterpret_cast<volatile double *>(sthr + kMaxWarps * 2);  // [2]: dt_max, K (bits)
+    uint32_t *hist = reinterpret_cast<uint32_t *>(const_cast<double *>(sinfo) + 2); // [RW][n_phi + 1][NT], 16-byte aligned
     const int hist_rows = EXT ? 2 * n_phi + 1 : n_phi + 1;  // EXT: a pair's shared floor(x) lets j reach 2 n_phi
     const uint32_t plane = (uint32_t)hist_rows * rs;                             // bytes per counter-word plane
     // shared-memory marginal (!REGM): RW planes of n_phi rows after the histogram; word (w2, j) of this thread is at
@@ -312,8 +334,6 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
     const int64_t tile_hi = prm.tiles_per_lc * (job + 1) / prm.jobs_per_lc;
     const int n_tiles = (int)(tile_hi - tile_lo);
     const int N = prm.info[lc].n;
-    const double dt_max = prm.info[lc].dt_max;
-    const int64_t K = prm.info[lc].K;
     const double2 *gpts = prm.pts + prm.lc_offsets[lc];
     const bool single = N <= prm.cap_points;            // the whole light curve stays resident for every tile
     const int CH = single ? N : prm.cap_points / 2;     // else: streamed through two half buffers, per tile
@@ -334,7 +354,12 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
     for (int i = tid; i < kLtabSmem; i += NT) sL[i] = i < prm.ltab_n ? prm.ltab[i] : 0;
     for (int i = tid; i <= n_m; i += NT) sseg[i] = prm.seg[(int64_t)lc * (n_m + 1) + i];
     if (tid < NW) stat_init(sstat + tid * kStatWords);
+    stop[2 * tid] = kInfS;
+    stop[2 * tid + 1] = kInfS;
+    if (tid < 2 * NW) sthr[tid] = kInfS;
     if (tid == 0) {
+        sinfo[0] = prm.info[lc].dt_max;
+        sinfo[1] = __longlong_as_double(prm.info[lc].K);
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -343,9 +368,6 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
             for (int g = 0; g < 2 && g < total_seq; ++g) issue_chunk(g);
     }
     __syncthreads();
-
-    WarpTopK top;
-    top.reset(prm.top_k > 0 ? prm.top_k : 1);
 
     const double nphi_d = (double)n_phi;
     const uint32_t negn = 0u - (uint32_t)n_phi;
@@ -385,30 +407,38 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
         }
         // ---- per-trial constants
         double invP[R], cc[R];  // SHARE_P: only invP[0] is used
-        int64_t qv[R];
-        bool valid[R];
         bool fast, pz;
-        trial_slot_constants<R, SHARE_P>(prm, s0, nphi_d, dt_max, invP, cc, qv, valid, fast, pz);
-        fast = __all_sync(0xffffffffu, fast);
-        pz = __all_sync(0xffffffffu, pz);
-        int org[R];  // trial (0..R-1, relative to s0) held by slot r
-#pragma unroll
-        for (int r = 0; r < R; ++r) org[r] = r;
-        bool pair_ok = EXT && fast && !pz, quad_ok = pair_ok;
-        if (EXT) {
-            sort_slots_by_c<R>(cc, qv, valid, org, dt_max, pair_ok, quad_ok);
-            pair_ok = __all_sync(0xffffffffu, pair_ok);
-            quad_ok = __all_sync(0xffffffffu, quad_ok);
-        }
+        uint32_t orgp = 0;  // 2 bits per slot: the trial (0..R-1, relative to s0) held by slot r (EXT sorts the slots by c)
+        bool pair_ok = false, quad_ok = false;
         int dpos[R];  // DUMP: position of the slot's trial in the caller's list
 #pragma unroll
         for (int r = 0; r < R; ++r) dpos[r] = -1;
-        if (DUMP) {
-            for (int64_t i = 0; i < prm.n_dump; ++i) {
-                const int64_t q = prm.trial_q[i];
+        {
+            int64_t qv[R];
+            bool valid[R];
+            int org[R];
+            const double dt_max = sinfo[0];
+            trial_slot_constants<R, SHARE_P>(prm, s0, nphi_d, dt_max, invP, cc, qv, valid, fast, pz);
+            fast = __all_sync(0xffffffffu, fast);
+            pz = __all_sync(0xffffffffu, pz);
 #pragma unroll
-                for (int r = 0; r < R; ++r)
-                    if (valid[r] && qv[r] == q) dpos[r] = (int)i;
+            for (int r = 0; r < R; ++r) org[r] = r;
+            pair_ok = EXT && fast && !pz;
+            quad_ok = pair_ok;
+            if (EXT) {
+                sort_slots_by_c<R>(cc, qv, valid, org, dt_max, pair_ok, quad_ok);
+                pair_ok = __all_sync(0xffffffffu, pair_ok);
+                quad_ok = __all_sync(0xffffffffu, quad_ok);
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) orgp |= (uint32_t)org[r] << (2 * r);
+            if (DUMP) {
+                for (int64_t i = 0; i < prm.n_dump; ++i) {
+                    const int64_t q = prm.trial_q[i];
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if (valid[r] && qv[r] == q) dpos[r] = (int)i;
+                }
             }
         }
 
@@ -431,6 +461,14 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
+#ifdef GCE_NOINLINE_FOLD
+                        if constexpr (R == 4 && SHARE_P && NPHI > 0) {
+                            if (pz) fold_range_call4<true, 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
+                            else if (EXT && quad_ok) fold_range_call4<false, EXT ? 2 : 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
+                            else if (EXT && pair_ok) fold_range_call4<false, EXT ? 1 : 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
+                            else fold_range_call4<false, 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
+                        } else
+#endif
                         if (pz) fold_range<R, SHARE_P, true, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
                         else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
                         else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
@@ -527,7 +565,7 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                     if (EXT) {
 #pragma unroll
                         for (int r = 0; r < R; ++r)
-                            if (org[r] == t) cet[t] = ce[r];
+                            if ((int)((orgp >> (2 * r)) & 3u) == t) cet[t] = ce[r];
                     }
                 }
                 if (R == 4 && !prm.ce_fp64 && s0 + R <= prm.n_trials && (reinterpret_cast<uintptr_t>(o32) & 15u) == 0) {
@@ -541,11 +579,27 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                     }
                 }
             }
+            // the slot's trial, recomputed here instead of being carried through the hot loop
+            int64_t qv[R];
+            bool valid[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int64_t s = s0 + (int64_t)(EXT ? ((orgp >> (2 * r)) & 3u) : (uint32_t)r);
+                valid[r] = s < prm.n_trials;
+                qv[r] = (valid[r] ? s : 0) + prm.q_off;
+            }
             if (prm.top_k > 0) {
+                volatile int64_t *vtop = stop + 2 * tid, *vthr = sthr + 2 * (tid >> 5);
+                WarpTopK top;
+                top.k = prm.top_k;
+                top.S = vtop[0]; top.q = vtop[1]; top.thrS = vthr[0]; top.thrq = vthr[1];
 #pragma unroll
                 for (int r = 0; r < R; ++r) top.offer((valid[r] && N > 0) ? S[r] : kInfS, (valid[r] && N > 0) ? qv[r] : kInfS);
+                vtop[0] = top.S; vtop[1] = top.q;
+                if (lane == 0) { vthr[0] = top.thrS; vthr[1] = top.thrq; }
             }
             if (prm.part_stats != nullptr && N > 0) {  // Eq. 5 partial sums of this tile, warp-reduced, exact integers
+                const int64_t K = __double_as_longlong(sinfo[1]);
                 __int128 a = 0;
                 u128_t b = 0;
                 int64_t mn = kInfS, mx = INT64_MIN;
@@ -589,21 +643,11 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
     // ---------------- per-CTA merge of the warps' top-k lists -> partial[lc][job][k]
     if (!DUMP && prm.top_k > 0) {
         const int K = prm.top_k;
-        __syncthreads();  // every issued TMA load has been consumed: the point buffer is idle, reuse it as scratch
-        int64_t *scr = reinterpret_cast<int64_t *>(spts);  // 16 * NW * K <= 10 KB <= cap_points * 16 (cap >= kMinPoints)
-        if (lane < K) {
-            scr[2 * ((tid >> 5) * K + lane)] = top.S;
-            scr[2 * ((tid >> 5) * K + lane) + 1] = top.q;
-        }
-        __syncthreads();
+        __syncthreads();  // the warps' lists in shared memory are final (lanes >= K hold +inf)
         if (tid < 32) {
+            WarpTopK top;
             top.reset(K);
-            for (int e = 0; e < NW * K; e += 32) {
-                const int i = e + lane;
-                const int64_t cS = i < NW * K ? scr[2 * i] : kInfS;
-                const int64_t cq = i < NW * K ? scr[2 * i + 1] : kInfS;
-                top.offer(cS, cq);
-            }
+            for (int w = 0; w < NW; ++w) top.offer(stop[2 * (w * 32 + lane)], stop[2 * (w * 32 + lane) + 1]);
             if (lane < K) {
                 const int64_t o = ((int64_t)lc * prm.jobs_per_lc + job) * K + lane;
                 prm.part_S[o] = top.S;
