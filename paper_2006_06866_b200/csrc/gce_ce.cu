@@ -78,12 +78,12 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     };
     int64_t nt_s = threads_beside(want_pts, false);
     if (nt_s > kMaxThreadsSmemMarg) nt_s = kMaxThreadsSmemMarg;
-    const bool regm_fits = templ && threads_beside(kMinPoints, true) >= kNtRegm;
-    // measured on C3: 512 threads with register marginals beat 608 threads with shared-memory
-    // marginals (83.7 vs 86.8 ms), so the register variant is taken whenever it fits
+    const bool regm_fits = templ && threads_beside(kMinPoints, true) >= nt_regm(n_phi);
+    // measured on C3: register marginals beat 608 threads with shared-memory marginals (83.7 vs
+    // 86.8 ms), so the register variant is taken whenever it fits; its thread count is per family (nt_regm)
     if (regm_fits) {
         p.regm = true;
-        p.nt = kNtRegm;
+        p.nt = nt_regm(n_phi);
     } else {
         p.regm = false;
         if (nt_s < 32) nt_s = threads_beside(kMinPoints, false);

@@ -89,10 +89,22 @@ constexpr int64_t kInfS = INT64_MAX;
 constexpr int kSmemLimit = 227 * 1024 - 8 * kLtabSmem;  // dynamic shared memory per CTA: 227 KB minus the static L table
 constexpr int kStatWords = 8;     // partial Eq. 5 sums: n, sum d (i128), sum d^2 (u192), min S, max S; d = S - K
 constexpr int kMaxWarps = 20;     // warps per CTA of the largest variant (640 threads)
-#ifndef GCE_NT_REGM
-#define GCE_NT_REGM 512
+// Threads per CTA of the register-marginal kernels (compile-time n_phi), per family.  512 threads = 4 warps per SM
+// sub-partition at <= 128 registers; 384 = 3 warps at <= 168.  n_phi = 30 keeps 60 marginal registers per thread: at
+// 128 the hot loop is starved of registers and at 384 threads it runs 4.6 % faster (measured on C5).
+#ifndef GCE_NT_N15
+#define GCE_NT_N15 512
 #endif
-constexpr int kNtRegm = GCE_NT_REGM;  // threads per CTA of the register-marginal kernels (compile-time n_phi)
+#ifndef GCE_NT_N20
+#define GCE_NT_N20 512
+#endif
+#ifndef GCE_NT_N30
+#define GCE_NT_N30 384
+#endif
+#ifndef GCE_NT_N50
+#define GCE_NT_N50 512
+#endif
+constexpr int nt_regm(int n_phi) { return n_phi == 15 ? GCE_NT_N15 : n_phi == 20 ? GCE_NT_N20 : n_phi == 30 ? GCE_NT_N30 : GCE_NT_N50; }
 constexpr int kCloseGroup = 5;    // phase bins whose read-and-clear atomics are in flight together in S4
 
 struct FalseT { static constexpr bool value = false; };

@@ -31,21 +31,21 @@ cudaError_t GCE_LAUNCHER_NAME(GCE_FAMILY, GCE_DUMP)(const SearchParams &sp, cons
 #elif GCE_FAMILY == 50
     // 50 phase bins (the paper's production binning): R = 2, the register marginal of 4 trials would take 100 registers
     if (!plan.regm || plan.ext || plan.R != 2) return cudaErrorInvalidValue;
-    if (plan.share_p) return launch_search<50, true, 2, true, D, false, kNtRegm>(sp, plan, n_lc, st);
-    return launch_search<50, true, 2, false, D, false, kNtRegm>(sp, plan, n_lc, st);
+    if (plan.share_p) return launch_search<50, true, 2, true, D, false, nt_regm(50)>(sp, plan, n_lc, st);
+    return launch_search<50, true, 2, false, D, false, nt_regm(50)>(sp, plan, n_lc, st);
 #else
     if (!plan.regm) return cudaErrorInvalidValue;
 #if GCE_FAMILY != 30
     if (plan.ext) {
         if (!plan.share_p || plan.R != 4) return cudaErrorInvalidValue;
-        return launch_search<N, true, 4, true, D, true, kNtRegm>(sp, plan, n_lc, st);
+        return launch_search<N, true, 4, true, D, true, nt_regm(N)>(sp, plan, n_lc, st);
     }
 #else
     if (plan.ext) return cudaErrorInvalidValue;
 #endif
-    if (plan.share_p && plan.R == 4) return launch_search<N, true, 4, true, D, false, kNtRegm>(sp, plan, n_lc, st);
-    if (plan.share_p && plan.R == 2) return launch_search<N, true, 2, true, D, false, kNtRegm>(sp, plan, n_lc, st);
-    if (!plan.share_p && plan.R == 4) return launch_search<N, true, 4, false, D, false, kNtRegm>(sp, plan, n_lc, st);
+    if (plan.share_p && plan.R == 4) return launch_search<N, true, 4, true, D, false, nt_regm(N)>(sp, plan, n_lc, st);
+    if (plan.share_p && plan.R == 2) return launch_search<N, true, 2, true, D, false, nt_regm(N)>(sp, plan, n_lc, st);
+    if (!plan.share_p && plan.R == 4) return launch_search<N, true, 4, false, D, false, nt_regm(N)>(sp, plan, n_lc, st);
     return cudaErrorInvalidValue;
 #endif
 }

@@ -140,9 +140,12 @@ def _fold_modes_of(gce, w, lc, qs):
 
 
 def _tile_edge_trials(n_trials, tile, rng, n_random):
-    """First / last trial, both sides of the first tile boundaries and of a boundary deep in the grid, plus a random sample."""
-    deep = (n_trials // tile // 2) * tile
-    edge = [0, 1, 3, 4, tile - 1, tile, tile + 1, 2 * tile - 1, 2 * tile, deep - 1, deep, deep + 5, n_trials - 2, n_trials - 1]
+    """First / last trial, both sides of the first tile boundaries and of a boundary deep in the grid, plus a random sample.
+    A tile is threads x trials-per-thread; the kernels run 512 or 384 threads, so the edges of both tilings are taken."""
+    edge = [0, 1, 3, 4, n_trials - 2, n_trials - 1]
+    for t in (tile, tile * 3 // 4):
+        deep = (n_trials // t // 2) * t
+        edge += [t - 1, t, t + 1, 2 * t - 1, 2 * t, deep - 1, deep, deep + 5]
     q = np.concatenate([np.array(edge), rng.integers(0, n_trials, size=n_random)])
     return np.unique(q[(q >= 0) & (q < n_trials)]).astype(np.int64)
 
@@ -163,7 +166,7 @@ def test_c3_full_counts_of_the_timed_kernel(gce, oracle):
 
 
 def test_c5_full_counts_of_the_timed_kernel(gce, oracle):
-    """configs[4] at full size: k_search<30,1,4,1,.,0,512> in dump mode, all 16 light curves of 5000 points (magnitude bins
+    """configs[4] at full size: k_search<30,1,4,1,.,0,384> in dump mode, all 16 light curves of 5000 points (magnitude bins
     above 1024 points: the table's global tail), counts bit-exact at tile edges and on a random sample."""
     w = W.make("C5")
     n_trials = w.periods.size * w.pdots.size
