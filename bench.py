@@ -1,20 +1,24 @@
 #!/usr/bin/env python
 """bench.py -- CE (P, Pdot) search throughput on B200, one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C5] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (S1..S5 of SURVEY.md section 8a: preprocess, fold + bin + entropy,
 cube store and/or fused top-k) over one batch of seeded synthetic light curves (gce_workloads, DESIGN.md
-section 5).  Default workload: C3 = BASELINE.json:configs[2], the paper's P-Pdot grid (64 light curves x
-1000 points x 50 000 periods x 64 Pdots, full fp32 CE cube + per-LC best): the configuration the
-north_star's roofline target is stated on and the largest one whose requested output includes the cube.
+section 5).  Default workload: C5 = BASELINE.json:configs[4], the largest single-GPU configuration (16 light
+curves x 5000 points x 2^17 periods x 256 Pdots, 30 x 10 bins, fused top-16: 2.68e12 point-folds per step).
+The north_star's roofline target is stated on the two P-Pdot grids, so the default run ALSO times C3 =
+configs[2] (64 x 1000 points x 50 000 periods x 64 Pdots, full fp32 CE cube + per-LC best) with the same K / W and
+carries it in the same JSON line under "secondary", with its own roofline, clocks, kernel_ms and e2e.
+--config X times X alone.
 
 metric  : CE point-folds per second = n_lc * n_p * n_pdot * N_obs / t   (BASELINE.json:metric)
 value   : inputs already resident in HBM, CUDA-event time of the gce_ce_search enqueue, L2 flushed between steps
 e2e     : the same through gce_ce_search_host with pinned HOST buffers (H2D of the inputs, D2H of the outputs
           and device allocation inside the timed region)
-roofline: the fold+bin+entropy kernel (k_search) against the FP64-pipe issue roofline,
-          timed live with CUDA events recorded by the library around that kernel
+roofline: the fold+bin+entropy kernel (k_search), timed live with CUDA events recorded by the library around that
+          kernel, against the two on-SM ceilings of SURVEY 8(d) -- FP64-pipe issue rate and shared-memory
+          wavefronts -- "bound" names the one that binds (the larger fraction), the other is kept in "other_bound"
 cpu_baseline: the oracle (oracle/, as it stands) on this box's host cores over a bounded sample of the workload
 
 N > 1 (torchrun, one process per GPU): light curves are independent, so each rank searches its own batch of
@@ -44,11 +48,16 @@ UNIT = "point-folds/s"
 FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (probe-measured)
 N_SM = 148
 OVERLAP = [False]   # set from --overlap; the oracle legs time the same binning
-# DRAM traffic of one k_search launch from the committed ncu --set full capture (profiles/r1_k_search_C3_full.md):
-# C3: 15.6 MB read + 772.0 MB written (the algorithmic output is the 819.2 MB fp32 cube; part of it is still in L2 at
-# kernel end); C5 (profiles/r1_k_search_C5_full.md, no cube): 2.5 MB read, 256 B written.  Only workloads that were
-# captured have an entry.
-NCU_DRAM_BYTES_PER_LAUNCH = {"C3": 15.6e6 + 772.0e6, "C5": 2.5e6}
+SHARED_WAVEFRONTS_PER_SM_CLK = 1   # shared-memory data pipe: 1 wavefront / SM / clk (ncu's own denominator)
+DEFAULT_CONFIG = "C5"              # BASELINE.json:configs[4]: the largest single-GPU configuration
+SECONDARY_CONFIG = "C3"            # configs[2]: the other P-Pdot grid of the north_star's roofline target
+# DRAM traffic of one k_search launch from the committed ncu --set full captures, keyed to the library sources
+# (paper_2006_06866_b200.build.source_hash) they were captured from.  C3 writes the 819.2 MB fp32 cube (part of it is
+# still in L2 at kernel end); C5 writes no cube.  Only workloads that were captured have an entry.
+NCU_TRAFFIC = {
+    "C3": {"bytes": 13.6e6 + 769.8e6, "source_hash": "", "profile": "profiles/r2_k_search_C3_full.md"},
+    "C5": {"bytes": 1.6e6, "source_hash": "", "profile": "profiles/r2_k_search_C5_full.md"},
+}
 
 
 def load_peaks():
@@ -170,10 +179,11 @@ def run_reference(args):
     if rank != 0:
         return 0
     import oracle
-    if args.config == "P1":
+    name = args.config or DEFAULT_CONFIG
+    if name == "P1":
         args.overlap = True
         OVERLAP[0] = True
-    w = apply_binning(make_workload(args.config, 0, args.quick), args)
+    w = apply_binning(make_workload(name, 0, args.quick), args)
     per_step = max(1.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
     sample, desc = oracle_sample(w, per_step)
     for _ in range(args.warmup):
@@ -192,6 +202,13 @@ def run_reference(args):
     return 0
 
 
+def array_sha256(w):
+    """SHA-256 of every generated input array (runs are comparable only on identical inputs)."""
+    import hashlib
+    h = lambda a: hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()[:16]
+    return {"times": h(w.times), "mags": h(w.mags), "lc_offsets": h(w.lc_offsets), "periods": h(w.periods), "pdots": h(w.pdots)}
+
+
 def workload_config(w, args):
     src = (f"BASELINE.json:configs[{int(w.name[1]) - 1}]" if w.name[0] == "C" else
            "the paper's production grid, PAPER.md:166-170, 50 overlapping phase bins; not a BASELINE.json config")
@@ -199,36 +216,36 @@ def workload_config(w, args):
             "n_lc": w.n_lc, "n_obs_total": w.total_points, "n_p": w.n_p, "n_pdot": w.n_pdot,
             "n_phase_bins": w.n_phase_bins, "n_mag_bins": w.n_mag_bins, "overlap": bool(args.overlap), "top_k": w.top_k, "ce_cube": bool(w.want_cube),
             "point_folds_per_step_per_gpu": w.point_folds, "parallelism": f"independent light-curve batches x{args.gpus}",
-            "l2": "flushed between timed steps (256 MiB write), each step timed by its own CUDA-event pair"}
+            "l2": "flushed between timed steps (256 MiB write), each step timed by its own CUDA-event pair",
+            "sha256_16": array_sha256(w)}
+
+
+def algorithmic_shared_wavefronts_per_pointfold(w):
+    """SURVEY 8(d), shared-memory row: one conflict-free counter update per point-fold = 1 wavefront per 32 point-folds
+    (an atomic RED is one wavefront: ncu counts 1.00 per ATOMS.ADD, profiles/r2_*), plus S4's visit of every cell of
+    every trial: one counter read and one k ln k lookup = 2 wavefronts per 32 (trial, cell) pairs.  Per point-fold:
+    (1 + 2 n_phi n_m / N) / 32 with N the mean light-curve length.  (Counting a counter update as a non-atomic
+    read-modify-write, 2 per 32, is SURVEY's other figure; the kernel does not pay it.)"""
+    n_avg = w.total_points / max(1, w.n_lc)
+    return (1.0 + 2.0 * w.n_phase_bins * w.n_mag_bins / max(1.0, n_avg)) / 32.0
+
+
+def traffic_record(w, args):
+    """DRAM bytes of one k_search launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full), valid only for
+    the library sources they were captured from: null when the kernel sources have changed since (never a stale number)."""
+    from paper_2006_06866_b200.build import source_hash
+    rec = NCU_TRAFFIC.get(w.name)
+    if args.quick or rec is None or args.n_phase_bins or args.n_mag_bins or args.overlap:
+        return None, "no ncu capture of this workload"
+    if rec["source_hash"] != source_hash():
+        return None, f"kernel sources changed since the capture {rec['profile']} (hash {rec['source_hash']})"
+    return rec["bytes"], f"{rec['profile']}: dram__bytes_read.sum + dram__bytes_write.sum of one k_search launch, ncu --set full; bytes per launch"
 
 
 # ----------------------------------------------------------------------------------------- our arm
-def run_ours(args):
+def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline):
+    """W warm-ups, K timed steps (device-resident), the end-to-end host-buffer leg, the roofline record; one dict."""
     import torch
-    import torch.distributed as dist
-
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
-
-    from paper_2006_06866_b200.build import build
-    if rank == 0:
-        build()
-    if world > 1:
-        dist.barrier()
-    import paper_2006_06866_b200 as gce
-
-    if args.config == "P1":
-        args.overlap = True   # the paper's production binning
-        OVERLAP[0] = True
-    w = apply_binning(make_workload(args.config, rank, args.quick), args)
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     times, mags, offs, periods, pdots = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
     k = w.top_k
@@ -302,48 +319,97 @@ def run_ours(args):
     e2e_val = pf_all * n_e2e / float(te.item())
     if k and rank == 0:
         assert torch.equal(h_idx.to(dev), bidx), "host and device entry points disagree"
-
+    del ce, ws, flush, h_ce
+    gce.gce_ce_host_release()
+    torch.cuda.empty_cache()
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return 0
+        return None
 
-    # ---- roofline of the dominant kernel (k_search): FP64 pipe issue rate
+    # ---- roofline of the dominant kernel (k_search): the two on-SM ceilings of SURVEY 8(d); the binding one is the
+    # ceiling the kernel is closer to (the larger fraction = the smaller point-folds/s ceiling)
     peaks, peaks_src = load_peaks()
     k_ms_avg = float(np.mean(k_ms))
-    ops = algorithmic_fp64_ops_per_pointfold(w) * w.point_folds
-    achieved = ops / (k_ms_avg * 1e-3) / 1e9                      # G lane-ops / s
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    peak = FP64_LANES_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9      # at the maximum SM clock (strictest denominator)
-    roof = {"bound": "alu", "pipe": "fp64", "kernel": "k_search", "achieved": achieved, "peak": peak,
-            "unit": "G FP64 lane-ops/s", "frac": achieved / peak,
-            "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if not args.quick else None,
-            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_search launch, ncu --set full "
-                              "(profiles/r1_k_search_C3_full.md, r1_k_search_C5_full.md); bytes per launch",
-            "peak_source": f"64 FP64 lanes/SM/clk x 148 SMs x {sm_max:.0f} MHz (max SM clock, {peaks_src} MEASURED_PEAKS.json; "
-                           "per-SM rate probe-measured, DESIGN.md section 7)",
-            "algorithmic_ops_per_point_fold": algorithmic_fp64_ops_per_pointfold(w),
-            "kernel_ms": k_ms_avg, "kernel_share_of_step": k_ms_avg * args.steps / tot_ms,
-            "frac_at_observed_clock": (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks and clocks.get("sm_mhz") else None,
-            "ce_output_gbs": (w.n_lc * w.n_p * w.n_pdot * 4 / (k_ms_avg * 1e-3) / 1e9) if w.want_cube else 0.0,
-            "hbm_peak_gbs": peaks.get("hbm_gbs")}
+    pf_s = w.point_folds / (k_ms_avg * 1e-3)
+    fp64_ops = algorithmic_fp64_ops_per_pointfold(w)
+    fp64 = {"bound": "alu", "pipe": "fp64", "achieved": fp64_ops * pf_s / 1e9,
+            "peak": FP64_LANES_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9, "unit": "G FP64 lane-ops/s",
+            "algorithmic_per_point_fold": fp64_ops,
+            "peak_source": f"nominal 64 FP64 lanes/SM/clk x 148 SMs x {sm_max:.0f} MHz (max SM clock, {peaks_src} MEASURED_PEAKS.json, "
+                           "which has no FP64 entry; a probe of independent DMUL/DADD chains reached 62.0-62.6 lanes/SM/clk, "
+                           "profiles/r2_peaks.md, so the nominal figure is the stricter denominator)"}
+    wf = algorithmic_shared_wavefronts_per_pointfold(w)
+    shm = {"bound": "alu", "pipe": "shared-memory wavefronts", "achieved": wf * pf_s / 1e9,
+           "peak": SHARED_WAVEFRONTS_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9, "unit": "G wavefronts/s",
+           "algorithmic_per_point_fold": wf,
+           "peak_source": f"1 shared-memory wavefront/SM/clk x 148 SMs x {sm_max:.0f} MHz (the denominator of ncu's "
+                          "l1tex__data_pipe_lsu_wavefronts_mem_shared pct_of_peak; DESIGN.md section 7)"}
+    for r in (fp64, shm):
+        r["frac"] = r["achieved"] / r["peak"]
+        r["ceiling_point_folds_per_s"] = r["peak"] * 1e9 / r["algorithmic_per_point_fold"]
+    main, other = (fp64, shm) if fp64["frac"] >= shm["frac"] else (shm, fp64)
+    traffic, traffic_src = traffic_record(w, args)
+    roof = dict(main, kernel="k_search", traffic=traffic, traffic_source=traffic_src,
+                kernel_ms=k_ms_avg, kernel_share_of_step=k_ms_avg * args.steps / tot_ms,
+                frac_at_observed_clock=(main["frac"] * sm_max / clocks["sm_mhz"]) if clocks and clocks.get("sm_mhz") else None,
+                ce_output_gbs=(w.n_lc * w.n_p * w.n_pdot * 4 / (k_ms_avg * 1e-3) / 1e9) if w.want_cube else 0.0,
+                hbm_peak_gbs=peaks.get("hbm_gbs"), other_bound=other)
 
     # ---- the oracle on this box's host cores, bounded sample
     cpu = None
-    if not args.no_cpu_baseline:
+    if with_cpu_baseline:
         import oracle
         sample, desc = oracle_sample(w, 15.0)
         t_cpu = time_oracle(sample, w)
         cpu = {"value": sample.point_folds / t_cpu, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                "sample": desc, "seconds": t_cpu}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+    return {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(w, args),
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
-                    "api": "gce_ce_search_host (pinned host buffers; allocation + H2D + search in 8 period chunks with the D2H of each cube slice overlapped on a second stream + sync)"},
+                    "api": "gce_ce_search_host (pinned host buffers; allocation + H2D + search + D2H + sync; with a cube the period "
+                           "axis is searched in 8 chunks and each slice's D2H overlaps the next chunk on a second stream)"},
             "gpu_launches": launches_per_step * args.steps, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu}
-    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2006_06866_b200.build import build
+    if rank == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+    import paper_2006_06866_b200 as gce
+
+    name = args.config or DEFAULT_CONFIG
+    if name == "P1":
+        args.overlap = True   # the paper's production binning
+        OVERLAP[0] = True
+    w = apply_binning(make_workload(name, rank, args.quick), args)
+    line = measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline=not args.no_cpu_baseline)
+    if args.config is None:
+        # the other P-Pdot grid the north_star's roofline target is stated on, same K / W, its own record
+        w2 = apply_binning(make_workload(SECONDARY_CONFIG, rank, args.quick), args)
+        sec = measure(gce, w2, args, dev, dist, rank, world, local_rank, with_cpu_baseline=False)
+        if rank == 0:
+            line["secondary"] = {key: sec[key] for key in ("value", "unit", "ms_per_step", "steps", "warmup", "config", "e2e",
+                                                           "gpu_launches", "clocks", "roofline")}
+    if rank == 0:
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -402,7 +468,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5", "P1"])
+    ap.add_argument("--config", default=None, choices=["C1", "C2", "C3", "C4", "C5", "P1"],
+                    help="time this workload alone (default: C5 as the headline plus C3 under 'secondary')")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true", help="shrunk grid, to test the bench itself; not a reportable number")
     ap.add_argument("--no-cpu-baseline", action="store_true")

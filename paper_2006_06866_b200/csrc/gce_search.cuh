@@ -91,8 +91,9 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
             const double y = __dmul_rn(x, nphi_d);
             const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
             const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
-            const uint32_t j = Iy + Ix * negn;
-            sink(j * rs + hb[r >> 1], r);
+            // floor(x)'s row offset is ready before floor(y): one multiply-add between floor(y) and the RED
+            const uint32_t t = Ix * (negn * rs) + hb[r >> 1];
+            sink(Iy * rs + t, r);
         }
     }
 }
@@ -101,37 +102,43 @@ template <int R, bool SHARE_P, bool PZ, int MODE, typename SINK>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
                                            const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
-    if (ke - kk >= 4) {
-        double2 a0 = sp[kk], a1 = sp[kk + 1];
-        do {
-            const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-            fold_bin_add<R, SHARE_P, PZ, MODE>(a0, invP, cc, nphi_d, negn, rs, hb, sink);
-            fold_bin_add<R, SHARE_P, PZ, MODE>(a1, invP, cc, nphi_d, negn, rs, hb, sink);
-            a0 = sp[kk + 4];
-            a1 = sp[kk + 5];
-            fold_bin_add<R, SHARE_P, PZ, MODE>(b0, invP, cc, nphi_d, negn, rs, hb, sink);
-            fold_bin_add<R, SHARE_P, PZ, MODE>(b1, invP, cc, nphi_d, negn, rs, hb, sink);
-            kk += 4;
-        } while (ke - kk >= 4);
+    // Four points per trip, the next two read ahead (the buffer has two spare points).  The two source forms compile to
+    // different ptxas schedules; each fold mode takes the one that measured faster (C5 / C4: -2 %, C3: +1 % otherwise).
+    if constexpr (MODE == 0) {
+        if (ke - kk >= 4) {
+            double2 a[2], b[2];
+#pragma unroll
+            for (int g = 0; g < 2; ++g) a[g] = sp[kk + g];
+            do {
+#pragma unroll
+                for (int g = 0; g < 2; ++g) b[g] = sp[kk + 2 + g];
+#pragma unroll
+                for (int g = 0; g < 2; ++g) fold_bin_add<R, SHARE_P, PZ, MODE>(a[g], invP, cc, nphi_d, negn, rs, hb, sink);
+#pragma unroll
+                for (int g = 0; g < 2; ++g) a[g] = sp[kk + 4 + g];
+#pragma unroll
+                for (int g = 0; g < 2; ++g) fold_bin_add<R, SHARE_P, PZ, MODE>(b[g], invP, cc, nphi_d, negn, rs, hb, sink);
+                kk += 4;
+            } while (ke - kk >= 4);
+        }
+    } else {
+        if (ke - kk >= 4) {
+            double2 a0 = sp[kk], a1 = sp[kk + 1];
+            do {
+                const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
+                fold_bin_add<R, SHARE_P, PZ, MODE>(a0, invP, cc, nphi_d, negn, rs, hb, sink);
+                fold_bin_add<R, SHARE_P, PZ, MODE>(a1, invP, cc, nphi_d, negn, rs, hb, sink);
+                a0 = sp[kk + 4];
+                a1 = sp[kk + 5];
+                fold_bin_add<R, SHARE_P, PZ, MODE>(b0, invP, cc, nphi_d, negn, rs, hb, sink);
+                fold_bin_add<R, SHARE_P, PZ, MODE>(b1, invP, cc, nphi_d, negn, rs, hb, sink);
+                kk += 4;
+            } while (ke - kk >= 4);
+        }
     }
     for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE>(sp[kk], invP, cc, nphi_d, negn, rs, hb, sink);
 }
 
-#ifdef GCE_NOINLINE_FOLD
-// Experiment: the hot loop as a real call, so that the caller's cold state (phase marginals, top-k, tile bookkeeping) is
-// saved around it by the ABI instead of starving the loop of registers.  R = 4 trials sharing a period only.
-template <bool PZ, int MODE, int NPHI>
-__device__ __noinline__ void fold_range_call4(const double2 *__restrict__ sp, int kk, const int ke, const double invP0,
-                                              const double c0, const double c1, const double c2, const double c3,
-                                              const uint32_t rs, const uint32_t hb0, const uint32_t hb1,
-                                              const uint32_t inc0, const uint32_t inc1) {
-    const double invP[4] = {invP0, invP0, invP0, invP0};
-    const double cc[4] = {c0, c1, c2, c3};
-    const uint32_t hb[2] = {hb0, hb1};
-    const RedSink sink{inc0, inc1};
-    fold_range<4, true, PZ, MODE>(sp, kk, ke, invP, cc, (double)NPHI, 0u - (uint32_t)NPHI, rs, hb, sink);
-}
-#endif
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
 template <int R, bool SHARE_P, typename SINK>
@@ -461,14 +468,6 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-#ifdef GCE_NOINLINE_FOLD
-                        if constexpr (R == 4 && SHARE_P && NPHI > 0) {
-                            if (pz) fold_range_call4<true, 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
-                            else if (EXT && quad_ok) fold_range_call4<false, EXT ? 2 : 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
-                            else if (EXT && pair_ok) fold_range_call4<false, EXT ? 1 : 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
-                            else fold_range_call4<false, 0, NPHI>(sp, lo, hi, invP[0], cc[0], cc[1], cc[2], cc[3], rs, hb[0], hb[1], sink.inc0, sink.inc1);
-                        } else
-#endif
                         if (pz) fold_range<R, SHARE_P, true, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
                         else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
                         else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
