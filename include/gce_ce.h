@@ -27,11 +27,13 @@
  *   - `times` need not be sorted.  `periods` are in the unit of `times`; `pdots` are dimensionless (s/s), any
  *     sign (:228).  Trials are addressed by the flat index q = ip * n_pdot + ipd.
  *   - Values that need device data to validate (non-monotone lc_offsets, P <= 0, non-finite inputs) are
- *     undefined behaviour on the device-pointer calls; gce_ce_validate_host checks host copies.  A light curve
- *     longer than GCE_CE_MAX_POINTS (GCE_CE_MAX_POINTS_OVERLAP with overlap = 1) is never folded with wrapped
- *     counters: the device-pointer calls return GCE_CE_ERR_RANGE when total_points alone proves it and
- *     otherwise treat that light curve as empty (CE = NaN, best index -1); the *_host calls, which see the
- *     offsets, return GCE_CE_ERR_RANGE.
+ *     undefined behaviour on the device-pointer calls; gce_ce_validate_host checks host copies.  Light curves of
+ *     any length up to GCE_CE_MAX_POINTS_WIDE are searched; beyond GCE_CE_MAX_POINTS (GCE_CE_MAX_POINTS_OVERLAP with
+ *     overlap = 1) the device-pointer caller must say so in gce_ce_params.max_lc_points (the lengths live on the
+ *     device; the *_host calls see the offsets and set it themselves).  A light curve longer than the call's limit
+ *     is never folded with wrapped counters: the device-pointer calls return GCE_CE_ERR_RANGE when total_points
+ *     alone proves it and otherwise treat that light curve as empty (CE = NaN, best index -1); the *_host calls
+ *     return GCE_CE_ERR_RANGE beyond GCE_CE_MAX_POINTS_WIDE.
  *   - A light curve with N = 0 yields CE = NaN for every trial and best index -1; N = 1 yields CE = 0.
  *   - There is no CPU fallback anywhere in this library.
  */
@@ -53,8 +55,10 @@ extern "C" {
 
 #define GCE_CE_MAX_BINS 64         /* n_phase_bins and n_mag_bins are each in 1..64                 */
 #define GCE_CE_MAX_TOPK 32         /* top_k is in 0..32                                             */
-#define GCE_CE_MAX_POINTS 65535    /* points per light curve (16-bit counters)                      */
+#define GCE_CE_MAX_FILTERS 8       /* filter ids are in 0..7 (normalise = 1)                        */
+#define GCE_CE_MAX_POINTS 65535    /* points per light curve with the default 16-bit counters       */
 #define GCE_CE_MAX_POINTS_OVERLAP 32767 /* ... with overlap = 1 (the table holds 2N entries)            */
+#define GCE_CE_MAX_POINTS_WIDE (1 << 26) /* ... of a call that announces longer light curves (max_lc_points) */
 
 typedef struct gce_ce_params {
     int32_t n_phase_bins; /* n_phi, 1..64                                                         */
@@ -65,11 +69,22 @@ typedef struct gce_ce_params {
     int32_t overlap;      /* 0: plain bins (hot path).  1: 50 % overlapping phase bins (:106, :162):
                            * n_phase_bins bins of width 2/n_phase_bins, bin k = plain cells k-1 and k (cyclic),
                            * every point counted twice, p = c / 2N.  The debug calls ignore it.            */
-    int32_t reserved[2];  /* must be 0                                                            */
+    int32_t max_lc_points; /* 0: every light curve has at most GCE_CE_MAX_POINTS (_OVERLAP) points.  Larger (up to
+                           * GCE_CE_MAX_POINTS_WIDE): an upper bound on the longest light curve of this call -- the
+                           * search then runs with 32-bit counters and a k ln k table of that length (the paper's
+                           * "base" variant for light curves of any length, :154).  gce_ce_search_host sets it itself. */
+    int32_t normalise;    /* 0: magnitudes are min/max-scaled per light curve (north_star, reading Q2).
+                           * 1: the paper's normalisation first (:96): per light curve and per filter, subtract the
+                           * median and divide by the standard deviation of that filter's magnitudes, so that the
+                           * filters can be merged into one light curve; the merged values are then min/max-binned as
+                           * before.  With one filter the bins equal those of normalise = 0 in exact arithmetic.     */
     /* Optional cudaEvent_t handles (NULL = none), recorded on `stream` immediately before / after the
      * fold+bin+entropy kernel, so a harness can time the dominant kernel alone without a profiler.    */
     void *ev_search_begin;
     void *ev_search_end;
+    /* normalise = 1 only: int32[total_points], the filter (0 .. GCE_CE_MAX_FILTERS - 1) of every point; NULL = all points
+     * belong to one filter.  A DEVICE pointer for the device-pointer calls, a HOST pointer for the *_host calls. */
+    const int32_t *filter_ids;
 } gce_ce_params;
 
 /* Bytes of device workspace gce_ce_search needs for these sizes (256-byte aligned base required).

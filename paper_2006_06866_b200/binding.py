@@ -6,6 +6,7 @@ the stream handle; nothing here computes.  There is no CPU fallback: if the libr
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 import os
 
@@ -20,7 +21,7 @@ if not os.path.exists(LIB):
 
 _lib = C.CDLL(LIB)
 
-MAX_BINS, MAX_TOPK, MAX_POINTS = 64, 32, 65535
+MAX_BINS, MAX_TOPK, MAX_POINTS, MAX_POINTS_OVERLAP, MAX_POINTS_WIDE = 64, 32, 65535, 32767, 1 << 26
 OK, ERR_POINTER, ERR_RANGE, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
 FOLD_AUTO, FOLD_PLAIN, FOLD_PAIR, FOLD_QUAD, FOLD_GENERIC, FOLD_PDOT_ZERO = range(6)   # gce_ce_debug_bins fold_mode
 
@@ -28,7 +29,8 @@ FOLD_AUTO, FOLD_PLAIN, FOLD_PAIR, FOLD_QUAD, FOLD_GENERIC, FOLD_PDOT_ZERO = rang
 class Params(C.Structure):
     _fields_ = [("n_phase_bins", C.c_int32), ("n_mag_bins", C.c_int32), ("top_k", C.c_int32),
                 ("ce_fp64", C.c_int32), ("want_stats", C.c_int32), ("overlap", C.c_int32),
-                ("reserved", C.c_int32 * 2), ("ev_search_begin", C.c_void_p), ("ev_search_end", C.c_void_p)]
+                ("max_lc_points", C.c_int32), ("normalise", C.c_int32), ("ev_search_begin", C.c_void_p),
+                ("ev_search_end", C.c_void_p), ("filter_ids", C.c_void_p)]
 
 
 _vp, _i32, _i64, _sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
@@ -82,13 +84,20 @@ def gce_ce_version() -> str:
 
 
 def make_params(n_phase_bins, n_mag_bins, top_k=0, ce_fp64=False, want_stats=False, overlap=False,
-                ev_search_begin=None, ev_search_end=None) -> Params:
+                ev_search_begin=None, ev_search_end=None, max_lc_points=0, normalise=False, filter_ids=None) -> Params:
     """ev_search_begin / ev_search_end: optional torch.cuda.Event(enable_timing=True) objects that have been
-    recorded at least once (torch creates the cudaEvent_t lazily); the caller keeps them alive."""
+    recorded at least once (torch creates the cudaEvent_t lazily).  max_lc_points: upper bound on the longest light
+    curve when that exceeds MAX_POINTS (32-bit counters).  normalise / filter_ids: the paper's per-filter median / std
+    normalisation; filter_ids is an int32 tensor [total_points] on the device (on the host for gce_ce_search_host)
+    or None.  The caller keeps the events and filter_ids alive."""
     def _ev(e):
         return None if e is None else C.c_void_p(e.cuda_event)
+    if filter_ids is not None:
+        if filter_ids.dtype != torch.int32 or not filter_ids.is_contiguous():
+            raise TypeError("filter_ids: contiguous int32 tensor expected")
     return Params(int(n_phase_bins), int(n_mag_bins), int(top_k), int(bool(ce_fp64)), int(bool(want_stats)),
-                  int(bool(overlap)), (C.c_int32 * 2)(0, 0), _ev(ev_search_begin), _ev(ev_search_end))
+                  int(bool(overlap)), int(max_lc_points), int(bool(normalise)), _ev(ev_search_begin), _ev(ev_search_end),
+                  None if filter_ids is None else C.c_void_p(filter_ids.data_ptr()))
 
 
 def gce_ce_workspace_bytes(total_points, n_lc, n_p, n_pdot, prm: Params) -> int:
@@ -282,9 +291,16 @@ class SearchResult:
 
 
 def search(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, top_k=0, want_cube=True,
-           ce_fp64=False, want_stats=False, overlap=False, workspace=None, stream=None) -> SearchResult:
-    """Allocate outputs + workspace with torch and call gce_ce_search (device tensors in, device tensors out)."""
-    prm = make_params(n_phase_bins, n_mag_bins, top_k, ce_fp64, want_stats, overlap)
+           ce_fp64=False, want_stats=False, overlap=False, workspace=None, stream=None, normalise=False,
+           filter_ids=None) -> SearchResult:
+    """Allocate outputs + workspace with torch and call gce_ce_search (device tensors in, device tensors out).
+    When the batch holds more points than one light curve may have with 16-bit counters, the longest light curve is read
+    back (one synchronisation) to announce it to the library (max_lc_points)."""
+    longest = 0
+    if times.numel() > (MAX_POINTS_OVERLAP if overlap else MAX_POINTS) and lc_offsets.numel() > 1:
+        longest = int((lc_offsets[1:] - lc_offsets[:-1]).max().item())
+    prm = make_params(n_phase_bins, n_mag_bins, top_k, ce_fp64, want_stats, overlap, max_lc_points=longest,
+                      normalise=normalise, filter_ids=filter_ids)
     dev = times.device
     n_lc = lc_offsets.numel() - 1
     n_p, n_pdot = periods.numel(), pdots.numel()
@@ -300,47 +316,58 @@ def search(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, to
 
 
 def search_period_chunks(times, mags, lc_offsets, periods, pdots, n_phase_bins, n_mag_bins, chunks, top_k=1,
-                         want_stats=True, overlap=False, ce_fp64=False, cube_sink=None, dist=None, stream=None) -> SearchResult:
+                         want_stats=True, overlap=False, ce_fp64=False, cube_sink=None, dist=None, stream=None,
+                         max_lc_points=0, normalise=False, filter_ids=None) -> SearchResult:
     """The search over a list of period ranges [(ip_begin, ip_end), ...] -- this process's share of the grid -- merged
     exactly (batches bound the memory, their minima are merged; period-axis split when
     there are fewer light curves than GPUs).  One workspace and one partial buffer are reused for every chunk.
-    cube_sink(ip_begin, ip_end, ce_slice) receives each cube slice [n_lc][ip_end - ip_begin][n_pdot] (device tensor,
-    overwritten by the next chunk) when given.  With `dist` (initialised torch.distributed, NCCL) the partial blobs of
+    cube_sink(ip_begin, ip_end, ce_slice) receives each non-empty cube slice [n_lc][ip_end - ip_begin][n_pdot] (device
+    tensor, overwritten by the next chunk) when given.  With `dist` (initialised torch.distributed) the partial blobs of
     all ranks are all-gathered -- n_lc x (2 top_k + 10) int64 per rank, the only exchange of the path -- and every rank
-    merges them, so every rank returns the whole grid's selection.  Argument marshalling and plumbing only: the merge
-    runs in the library's kernels."""
-    prm = make_params(n_phase_bins, n_mag_bins, top_k, ce_fp64, want_stats, overlap)
+    merges them, so every rank returns the whole grid's selection.  NCCL gathers the device blobs in stream order; a
+    backend without CUDA support (gloo) gets them staged through the host (kilobytes).  Argument marshalling and
+    plumbing only: the merge runs in the library's kernels."""
+    prm = make_params(n_phase_bins, n_mag_bins, top_k, ce_fp64, want_stats, overlap, max_lc_points=max_lc_points,
+                      normalise=normalise, filter_ids=filter_ids)
     dev = times.device
     n_lc = lc_offsets.numel() - 1
     n_pdot = pdots.numel()
     words = gce_ce_partial_words(top_k)
     chunks = [(int(a), int(b)) for a, b in chunks]
     widest = max([b - a for a, b in chunks], default=0)
-    ws = torch.empty(gce_ce_workspace_bytes(times.numel(), n_lc, widest, n_pdot, prm), dtype=torch.uint8, device=dev)
-    parts = torch.empty((max(len(chunks), 1), n_lc, words), dtype=torch.int64, device=dev)
-    ce = None
-    if cube_sink is not None and widest > 0:
-        ce = torch.empty(n_lc * widest * n_pdot, dtype=torch.float64 if ce_fp64 else torch.float32, device=dev)
-    if not chunks:  # a rank with no periods still contributes a (neutral) blob
-        gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm, 0, 0, parts[0], None, ws, stream)
-    for i, (a, b) in enumerate(chunks):
-        sl = ce[: n_lc * (b - a) * n_pdot] if ce is not None else None
-        gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm, a, b, parts[i], sl, ws, stream)
-        if cube_sink is not None:
-            cube_sink(a, b, sl.view(n_lc, b - a, n_pdot))
-    n_parts = parts.shape[0]
-    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
-        # ranks may hold different numbers of chunks: merge locally first, then exchange one blob array per rank
-        local = torch.empty((1, n_lc, words), dtype=torch.int64, device=dev)
-        _merge_to_partial(parts, n_parts, n_lc, prm, local, stream)
-        gathered = [torch.empty_like(local) for _ in range(dist.get_world_size())]
-        dist.all_gather(gathered, local)
-        parts = torch.cat(gathered, dim=0)
+    # everything below is ordered on `stream`: torch allocations, the collective and the library's kernels alike
+    with torch.cuda.stream(stream) if stream is not None else contextlib.nullcontext():
+        ws = torch.empty(gce_ce_workspace_bytes(times.numel(), n_lc, widest, n_pdot, prm), dtype=torch.uint8, device=dev)
+        parts = torch.empty((max(len(chunks), 1), n_lc, words), dtype=torch.int64, device=dev)
+        ce = None
+        if cube_sink is not None and widest > 0:
+            ce = torch.empty(n_lc * widest * n_pdot, dtype=torch.float64 if ce_fp64 else torch.float32, device=dev)
+        if not chunks:  # a rank with no periods still contributes a (neutral) blob
+            gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm, 0, 0, parts[0], None, ws, stream)
+        for i, (a, b) in enumerate(chunks):
+            sl = ce[: n_lc * (b - a) * n_pdot] if (ce is not None and b > a) else None
+            gce_ce_search_partial(times, mags, lc_offsets, periods, pdots, prm, a, b, parts[i], sl, ws, stream)
+            if cube_sink is not None and sl is not None:
+                cube_sink(a, b, sl.view(n_lc, b - a, n_pdot))
         n_parts = parts.shape[0]
-    bidx = torch.empty((n_lc, top_k), dtype=torch.int64, device=dev) if top_k > 0 else None
-    bce = torch.empty((n_lc, top_k), dtype=torch.float32, device=dev) if top_k > 0 else None
-    stats = torch.empty((n_lc, 4), dtype=torch.float64, device=dev) if want_stats else None
-    gce_ce_merge_partials(parts, n_parts, n_lc, prm, bidx, bce, stats, stream)
+        if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+            # ranks may hold different numbers of chunks: merge locally first, then exchange one blob array per rank
+            local = torch.empty((1, n_lc, words), dtype=torch.int64, device=dev)
+            _merge_to_partial(parts, n_parts, n_lc, prm, local, stream)
+            if str(dist.get_backend()) == "nccl":
+                gathered = [torch.empty_like(local) for _ in range(dist.get_world_size())]
+                dist.all_gather(gathered, local)
+                parts = torch.cat(gathered, dim=0)
+            else:
+                host = local.cpu()  # synchronises this stream
+                gathered = [torch.empty_like(host) for _ in range(dist.get_world_size())]
+                dist.all_gather(gathered, host)
+                parts = torch.cat(gathered, dim=0).to(dev)
+            n_parts = parts.shape[0]
+        bidx = torch.empty((n_lc, top_k), dtype=torch.int64, device=dev) if top_k > 0 else None
+        bce = torch.empty((n_lc, top_k), dtype=torch.float32, device=dev) if top_k > 0 else None
+        stats = torch.empty((n_lc, 4), dtype=torch.float64, device=dev) if want_stats else None
+        gce_ce_merge_partials(parts, n_parts, n_lc, prm, bidx, bce, stats, stream)
     return SearchResult(None, bidx, bce, stats)
 
 

@@ -46,9 +46,24 @@ size_t search_smem_fixed() {  // mbarriers, seg row, Eq. 5 accumulators, the war
 }
 // counter rows of one thread: histogram (n_phi + 1 rows, the last one catches RN(x * n_phi) == n_phi * (floor(x) + 1)),
 // plus n_phi marginal rows when the marginal is not in registers; RW words each
-size_t search_smem_per_thread(int n_phi, int R, bool regm, bool ext = false) {
+size_t search_smem_per_thread(int n_phi, int R, bool regm, bool ext = false, bool wide = false) {
     const int hist_rows = ext ? 2 * n_phi + 1 : n_phi + 1;
-    return (size_t)((R + 1) / 2) * (size_t)(regm ? hist_rows : hist_rows + n_phi) * sizeof(uint32_t);
+    return (size_t)(wide ? R : (R + 1) / 2) * (size_t)(regm ? hist_rows : hist_rows + n_phi) * sizeof(uint32_t);
+}
+
+// Points per light curve this call accepts, and whether it needs the 32-bit counters: the 16-bit range unless the
+// caller has announced longer light curves (gce_ce_params.max_lc_points).
+int64_t narrow_limit(const gce_ce_params *prm) { return prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS; }
+bool is_wide(const gce_ce_params *prm) { return (int64_t)prm->max_lc_points > narrow_limit(prm); }
+int64_t points_limit(const gce_ce_params *prm) { return is_wide(prm) ? (int64_t)prm->max_lc_points : narrow_limit(prm); }
+
+// Fixed-point shift of the k ln k table: 2^-42 for tables of up to 2^17 entries (every narrow call), else the largest
+// shift that keeps L(k_max) -- and with it every sum of table entries of one trial, which is at most L(k_max) -- below 2^61.
+int table_shift(int64_t ltab_n) {
+    const double kmax = (double)(ltab_n - 1);
+    if (kmax <= 131070.0) return kLfixShift;
+    const int bits = (int)ceil(log2(kmax * log(kmax)));
+    return 61 - bits;
 }
 
 // Trials per thread and whether they share a period: from the grid shape alone (also used by gce_ce_debug_bins).
@@ -61,11 +76,12 @@ void plan_trials(int64_t n_pdot, int n_phi, int *R, bool *share_p) {
     if (n_phi == 50) { *R = 2; *share_p = (n_pdot % 2 == 0); }
 }
 
-Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_pdot, int n_phi) {
+Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_pdot, int n_phi, bool wide) {
     Plan p;
-    plan_trials(n_pdot, n_phi, &p.R, &p.share_p);
+    p.wide = wide;
+    plan_trials(n_pdot, wide ? 0 : n_phi, &p.R, &p.share_p);
     const int64_t avail = (int64_t)kSmemLimit - (int64_t)search_smem_fixed();
-    const bool templ = n_phi == 15 || n_phi == 20 || n_phi == 30 || n_phi == 50;
+    const bool templ = !wide && (n_phi == 15 || n_phi == 20 || n_phi == 30 || n_phi == 50);  // wide counters: generic family
     // point buffer wanted: the average light curve plus a quarter (the per-LC lengths live on the device; a longer
     // light curve is streamed through the buffer in two halves instead of staying resident)
     const int64_t avg = n_lc > 0 ? (total_points + n_lc - 1) / n_lc : 0;
@@ -73,7 +89,7 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     if (want_pts < kMinPoints) want_pts = kMinPoints;
     if (want_pts > 8192) want_pts = 8192;
     auto threads_beside = [&](int64_t pts, bool regm) {
-        int64_t nt = (avail - (pts + 2) * (int64_t)sizeof(double2)) / (int64_t)search_smem_per_thread(n_phi, p.R, regm);
+        int64_t nt = (avail - (pts + 2) * (int64_t)sizeof(double2)) / (int64_t)search_smem_per_thread(n_phi, p.R, regm, false, wide);
         return nt < 0 ? 0 : nt / 32 * 32;
     };
     int64_t nt_s = threads_beside(want_pts, false);
@@ -95,7 +111,7 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     // 20 with R = 4 trials sharing a period; taken when the whole average light curve still fits beside the counters
     p.ext = p.regm && p.share_p && p.R == 4 && (n_phi == 15 || n_phi == 20) && n_pdot > 1 &&
             (avail - (int64_t)search_smem_per_thread(n_phi, p.R, true, true) * p.nt) / (int64_t)sizeof(double2) - 2 >= want_pts;
-    const int64_t planes = (int64_t)search_smem_per_thread(n_phi, p.R, p.regm, p.ext) * p.nt;
+    const int64_t planes = (int64_t)search_smem_per_thread(n_phi, p.R, p.regm, p.ext, wide) * p.nt;
     int64_t cap = (avail - planes) / (int64_t)sizeof(double2) - 2;  // - 2: read-ahead slack of the hot loop
     cap = cap / 8 * 8;
     if (cap > 8192) cap = 8192;  // 128 KB of points; longer light curves are streamed
@@ -123,11 +139,13 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     L.pts = o; o = align_up(o + sizeof(double2) * (size_t)(total_points > 0 ? total_points : 1), 256);
     L.seg = o; o = align_up(o + sizeof(int32_t) * (size_t)(n_lc > 0 ? n_lc : 1) * (prm->n_mag_bins + 1), 256);
     L.info = o; o = align_up(o + sizeof(LcInfo) * (size_t)(n_lc > 0 ? n_lc : 1), 256);
-    int64_t tn = (prm->overlap ? 2 : 1) * total_points;  // largest count looked up: N, or 2N with overlapping bins
-    if (tn > GCE_CE_MAX_POINTS) tn = GCE_CE_MAX_POINTS;
+    // largest count looked up: the longest light curve's N, or 2N with overlapping bins
+    int64_t longest = total_points < points_limit(prm) ? total_points : points_limit(prm);
+    int64_t tn = (prm->overlap ? 2 : 1) * longest;
+    if (!is_wide(prm) && tn > GCE_CE_MAX_POINTS) tn = GCE_CE_MAX_POINTS;
     L.ltab_n = (int)tn + 1;
     L.ltab = o; o = align_up(o + sizeof(int64_t) * (size_t)L.ltab_n, 256);
-    const Plan p = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins);
+    const Plan p = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins, is_wide(prm));
     const size_t parts = (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc * (size_t)(prm->top_k > 0 ? prm->top_k : 1);
     L.part_S = o; o = align_up(o + sizeof(int64_t) * parts, 256);
     L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
@@ -145,7 +163,8 @@ int check_params(const gce_ce_params *prm) {
     if (prm->ce_fp64 != 0 && prm->ce_fp64 != 1) return GCE_CE_ERR_RANGE;
     if (prm->want_stats != 0 && prm->want_stats != 1) return GCE_CE_ERR_RANGE;
     if (prm->overlap != 0 && prm->overlap != 1) return GCE_CE_ERR_RANGE;
-    if (prm->reserved[0] != 0 || prm->reserved[1] != 0) return GCE_CE_ERR_RANGE;
+    if (prm->max_lc_points < 0 || prm->max_lc_points > GCE_CE_MAX_POINTS_WIDE) return GCE_CE_ERR_RANGE;
+    if (prm->normalise != 0 && prm->normalise != 1) return GCE_CE_ERR_RANGE;
     return GCE_CE_OK;
 }
 
@@ -159,12 +178,23 @@ int check_sizes(int32_t n_lc, int64_t total_points, int64_t n_p, int64_t n_pdot)
 // Light-curve lengths from a HOST copy of lc_offsets: non-negative and within the counter range.
 int check_lengths_host(const int64_t *lc_offsets, int32_t n_lc, const gce_ce_params *prm) {
     if (n_lc > 0 && lc_offsets[0] != 0) return GCE_CE_ERR_RANGE;
-    const int64_t lim = prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS;
+    const int64_t lim = points_limit(prm);
     for (int32_t l = 0; l < n_lc; ++l) {
         const int64_t n = lc_offsets[l + 1] - lc_offsets[l];
         if (n < 0 || n > lim) return GCE_CE_ERR_RANGE;
     }
     return GCE_CE_OK;
+}
+
+// Host entries: raise max_lc_points to the longest light curve when that is beyond the 16-bit range.
+void host_set_max_lc_points(const int64_t *lc_offsets, int32_t n_lc, gce_ce_params *prm) {
+    int64_t longest = 0;
+    for (int32_t l = 0; l < n_lc; ++l) {
+        const int64_t n = lc_offsets[l + 1] - lc_offsets[l];
+        if (n > longest) longest = n;
+    }
+    if (longest > narrow_limit(prm) && longest <= GCE_CE_MAX_POINTS_WIDE && longest > (int64_t)prm->max_lc_points)
+        prm->max_lc_points = (int32_t)longest;
 }
 
 int cuda_fail(cudaError_t e) {
@@ -253,7 +283,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
         }
     }
     // more points than every light curve could hold within the counter range: some light curve must be too long
-    const int64_t max_points = prm->overlap ? GCE_CE_MAX_POINTS_OVERLAP : GCE_CE_MAX_POINTS;
+    const int64_t max_points = points_limit(prm);
     if (total_points > (int64_t)n_lc * max_points) return GCE_CE_ERR_RANGE;
     const int64_t n_trials = n_p * n_pdot;
     const int mult = prm->overlap ? 2 : 1;
@@ -268,7 +298,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     LcInfo *info = reinterpret_cast<LcInfo *>(ws + L.info);
     int64_t *ltab = reinterpret_cast<int64_t *>(ws + L.ltab);
 
-    const Plan plan = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins);
+    const Plan plan = make_plan(n_lc, total_points, n_trials, n_pdot, prm->n_phase_bins, is_wide(prm));
     SearchParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.pts = pts; sp.seg = seg; sp.info = info; sp.lc_offsets = lc_offsets; sp.ltab = ltab;
@@ -290,7 +320,7 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.out_counts = out_counts; sp.out_ce_at = out_ce_at;
 
     k_preprocess<<<n_lc + (L.ltab_n + 255) / 256, 256, 0, st>>>(times, mags, lc_offsets, n_lc, prm->n_mag_bins, pts, seg, info,
-                                                              ltab, L.ltab_n, mult, (int)max_points);
+                                                              ltab, L.ltab_n, table_shift(L.ltab_n), mult, (int)max_points);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     if (prm->ev_search_begin) {
@@ -443,12 +473,15 @@ int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc
 
 int gce_ce_validate_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                          const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                         const gce_ce_params *prm) {
-    int rc = check_params(prm);
+                         const gce_ce_params *prm_in) {
+    int rc = check_params(prm_in);
     if (rc) return rc;
     if (!lc_offsets) return GCE_CE_ERR_POINTER;
     if (n_lc < 0 || n_p < 0 || n_pdot < 1) return GCE_CE_ERR_RANGE;
     if (lc_offsets[0] != 0) return GCE_CE_ERR_RANGE;
+    gce_ce_params prm_local = *prm_in;  // what gce_ce_search_host would accept: lengths up to GCE_CE_MAX_POINTS_WIDE
+    host_set_max_lc_points(lc_offsets, n_lc, &prm_local);
+    const gce_ce_params *prm = &prm_local;
     rc = check_lengths_host(lc_offsets, n_lc, prm);
     if (rc) return rc;
     const int64_t total = lc_offsets[n_lc];
@@ -615,11 +648,14 @@ static int search_host_pipelined(const double *times, const double *mags, const 
 
 int gce_ce_search_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                        const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                       const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                       const gce_ce_params *prm_in, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
                        double *out_stats) {
-    int rc = check_params(prm);
+    int rc = check_params(prm_in);
     if (rc) return rc;
     if (!lc_offsets || n_lc < 0) return GCE_CE_ERR_POINTER;
+    gce_ce_params prm_local = *prm_in;
+    host_set_max_lc_points(lc_offsets, n_lc, &prm_local);  // the host entry sees the lengths: longer light curves -> 32-bit counters
+    const gce_ce_params *prm = &prm_local;
     const int64_t total = lc_offsets[n_lc];
     rc = check_sizes(n_lc, total, n_p, n_pdot);
     if (rc) return rc;

@@ -5,24 +5,25 @@
 
 namespace {
 
-// L(k) = k ln k in 2^-42 fixed point (k < 2^16 -> L < 2^62, and sum_j L(n_j) <= L(N), so the sums fit in int64).
-__device__ __forceinline__ int64_t ltab_entry(int k) {
-    return k < 2 ? 0 : __double2ll_rn(ldexp((double)k * log((double)k), kLfixShift));
+// L(k) = k ln k in 2^-shift fixed point.  shift = 42 for k < 2^17 (L < 2^62, and sum_j L(n_j) <= L(N), so the sums fit in
+// int64); longer tables (32-bit counters) take the smaller shift table_shift() chooses.
+__device__ __forceinline__ int64_t ltab_entry(int k, int shift) {
+    return k < 2 ? 0 : __double2ll_rn(ldexp((double)k * log((double)k), shift));
 }
 
 // ------------------------------------------------------------------------------------------------ S1
 // CTAs 0 .. n_lc-1: one per light curve.  Output points are permuted so equal magnitude bins are contiguous (counts do
 // not depend on point order); seg[lc][i] is the first point of magnitude bin i, seg[lc][n_m] = N.
 // CTAs n_lc ..: 256 entries each of the table L(k), k < ltab_n, that S4 looks up (one launch less than a kernel of its own).
-// A light curve longer than max_points (the 16-bit counters of k_search) is marked empty: CE = NaN, best index -1.
+// A light curve longer than max_points (the counter range of this call's k_search) is marked empty: CE = NaN, best index -1.
 __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ times, const double *__restrict__ mags,
                                                     const int64_t *__restrict__ lc_offsets, const int n_lc, const int n_m,
                                                     double2 *__restrict__ pts, int32_t *__restrict__ seg,
                                                     LcInfo *__restrict__ info, int64_t *__restrict__ ltab, const int ltab_n,
-                                                    const int mult, const int max_points) {
+                                                    const int lshift, const int mult, const int max_points) {
     if ((int)blockIdx.x >= n_lc) {
         const int k = ((int)blockIdx.x - n_lc) * 256 + (int)threadIdx.x;
-        if (k < ltab_n) ltab[k] = ltab_entry(k);
+        if (k < ltab_n) ltab[k] = ltab_entry(k, lshift);
         return;
     }
     __shared__ MinMax3 sh_red[8];
@@ -33,7 +34,7 @@ __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ t
     const int64_t n64 = lc_offsets[lc + 1] - off;
     if (n64 < 0 || n64 > (int64_t)max_points) {  // uniform per CTA
         for (int i = threadIdx.x; i <= n_m; i += blockDim.x) seg[(int64_t)lc * (n_m + 1) + i] = 0;
-        if (threadIdx.x == 0) info[lc] = LcInfo{0, 1, 0.0, 0};  // pad = 1: rejected
+        if (threadIdx.x == 0) info[lc] = LcInfo{0, lshift, 0.0, 0};  // rejected: treated as empty
         return;
     }
     const int n = (int)n64;
@@ -56,18 +57,18 @@ __global__ void __launch_bounds__(256) k_preprocess(const double *__restrict__ t
     __syncthreads();
     if (threadIdx.x == 0) {
         int acc = 0;
-        int64_t K = ltab_entry(mult * n);  // mult = 2 with overlapping phase bins: every point is counted twice
+        int64_t K = ltab_entry(mult * n, lshift);  // mult = 2 with overlapping phase bins: every point is counted twice
         for (int i = 0; i < n_m; ++i) {
             const int c = sh_cnt[i];
             seg[(int64_t)lc * (n_m + 1) + i] = acc;
             sh_cur[i] = acc;
             acc += c;
-            K -= ltab_entry(mult * c);
+            K -= ltab_entry(mult * c, lshift);
         }
         info[lc].K = K;
         seg[(int64_t)lc * (n_m + 1) + n_m] = acc;
         info[lc].n = n;
-        info[lc].pad = 0;
+        info[lc].lshift = lshift;
         info[lc].dt_max = n > 0 ? __dsub_rn(v.tmax, t0) : 0.0;
     }
     __syncthreads();

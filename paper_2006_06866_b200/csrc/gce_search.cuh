@@ -38,6 +38,14 @@ __device__ __forceinline__ void ltab_pair(const int64_t *__restrict__ sL, const 
     }
 }
 
+// WIDE counters (one 32-bit counter per trial, light curves beyond the 16-bit range): plain count, any size.
+__device__ __forceinline__ int64_t ltab_one(const int64_t *__restrict__ sL, const int64_t *__restrict__ gL, const uint32_t c) {
+    return c < (uint32_t)kLtabSmem ? sL[c] : gL[c];
+}
+
+// Counter words per thread: two 16-bit counters per word (WSH = 1) or one 32-bit counter per word (WSH = 0, WIDE).
+__host__ __device__ constexpr int n_words(int R, int WSH) { return WSH ? (R + 1) / 2 : R; }
+
 // S2 + S3 for one point and the R trials of this thread (DESIGN.md section 3; PAPER.md:100 Eq. 3, :106).
 //   a = dt*invP ; b = dt2*c ; x = a + b ; y = x*n_phi          (RN each, never fused)
 //   j = floor(y) - n_phi*floor(x)                               two exact round-down magic adds, |y| < 2^51
@@ -59,14 +67,14 @@ struct RedSink {
     __device__ __forceinline__ void operator()(const uint32_t addr, const int r) const { red_add_u32(addr, (r & 1) ? inc1 : inc0); }
 };
 
-template <int R, bool SHARE_P, bool PZ, int MODE, typename SINK>
+template <int R, bool SHARE_P, bool PZ, int MODE, int WSH = 1, typename SINK>
 __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&invP)[R], const double (&cc)[R],
                                              const double nphi_d, const uint32_t negn, const uint32_t rs,
-                                             const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
+                                             const uint32_t (&hb)[n_words(R, WSH)], const SINK &sink) {
     double a;
     if (SHARE_P) a = __dmul_rn(p.x, invP[0]);
     if constexpr (MODE != 0) {
-        static_assert(MODE == 0 || (SHARE_P && !PZ && R % 2 == 0), "shared floors need one period and Pdot != 0");
+        static_assert(MODE == 0 || (SHARE_P && !PZ && R % 2 == 0 && WSH == 1), "shared floors need one period, Pdot != 0 and packed counters");
         double x[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = __dadd_rn(a, __dmul_rn(p.y, cc[r]));
@@ -92,16 +100,16 @@ __device__ __forceinline__ void fold_bin_add(const double2 p, const double (&inv
             const uint32_t Iy = (uint32_t)__double2loint(__dadd_rd(y, kMagic));
             const uint32_t Ix = (uint32_t)__double2loint(__dadd_rd(x, kMagic));
             // floor(x)'s row offset is ready before floor(y): one multiply-add between floor(y) and the RED
-            const uint32_t t = Ix * (negn * rs) + hb[r >> 1];
+            const uint32_t t = Ix * (negn * rs) + hb[r >> WSH];
             sink(Iy * rs + t, r);
         }
     }
 }
 
-template <int R, bool SHARE_P, bool PZ, int MODE, typename SINK>
+template <int R, bool SHARE_P, bool PZ, int MODE, int WSH = 1, typename SINK>
 __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int kk, const int ke, const double (&invP)[R],
                                            const double (&cc)[R], const double nphi_d, const uint32_t negn,
-                                           const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
+                                           const uint32_t rs, const uint32_t (&hb)[n_words(R, WSH)], const SINK &sink) {
     // Four points per trip, the next two read ahead (the buffer has two spare points).  The two source forms compile to
     // different ptxas schedules; each fold mode takes the one that measured faster (C5 / C4: -2 %, C3: +1 % otherwise).
     if constexpr (MODE == 0) {
@@ -113,11 +121,11 @@ __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int k
 #pragma unroll
                 for (int g = 0; g < 2; ++g) b[g] = sp[kk + 2 + g];
 #pragma unroll
-                for (int g = 0; g < 2; ++g) fold_bin_add<R, SHARE_P, PZ, MODE>(a[g], invP, cc, nphi_d, negn, rs, hb, sink);
+                for (int g = 0; g < 2; ++g) fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(a[g], invP, cc, nphi_d, negn, rs, hb, sink);
 #pragma unroll
                 for (int g = 0; g < 2; ++g) a[g] = sp[kk + 4 + g];
 #pragma unroll
-                for (int g = 0; g < 2; ++g) fold_bin_add<R, SHARE_P, PZ, MODE>(b[g], invP, cc, nphi_d, negn, rs, hb, sink);
+                for (int g = 0; g < 2; ++g) fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(b[g], invP, cc, nphi_d, negn, rs, hb, sink);
                 kk += 4;
             } while (ke - kk >= 4);
         }
@@ -126,36 +134,36 @@ __device__ __forceinline__ void fold_range(const double2 *__restrict__ sp, int k
             double2 a0 = sp[kk], a1 = sp[kk + 1];
             do {
                 const double2 b0 = sp[kk + 2], b1 = sp[kk + 3];
-                fold_bin_add<R, SHARE_P, PZ, MODE>(a0, invP, cc, nphi_d, negn, rs, hb, sink);
-                fold_bin_add<R, SHARE_P, PZ, MODE>(a1, invP, cc, nphi_d, negn, rs, hb, sink);
+                fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(a0, invP, cc, nphi_d, negn, rs, hb, sink);
+                fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(a1, invP, cc, nphi_d, negn, rs, hb, sink);
                 a0 = sp[kk + 4];
                 a1 = sp[kk + 5];
-                fold_bin_add<R, SHARE_P, PZ, MODE>(b0, invP, cc, nphi_d, negn, rs, hb, sink);
-                fold_bin_add<R, SHARE_P, PZ, MODE>(b1, invP, cc, nphi_d, negn, rs, hb, sink);
+                fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(b0, invP, cc, nphi_d, negn, rs, hb, sink);
+                fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(b1, invP, cc, nphi_d, negn, rs, hb, sink);
                 kk += 4;
             } while (ke - kk >= 4);
         }
     }
-    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE>(sp[kk], invP, cc, nphi_d, negn, rs, hb, sink);
+    for (; kk < ke; ++kk) fold_bin_add<R, SHARE_P, PZ, MODE, WSH>(sp[kk], invP, cc, nphi_d, negn, rs, hb, sink);
 }
 
 
 // Rare path (|y| >= 2^51 for some point): the listing of DESIGN.md section 3 with 64-bit integers.
-template <int R, bool SHARE_P, typename SINK>
+template <int R, bool SHARE_P, int WSH = 1, typename SINK>
 __device__ __forceinline__ void fold_bin_add_generic(const double2 p, const double (&invP)[R], const double (&cc)[R],
-                                                     const int n_phi, const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2],
+                                                     const int n_phi, const uint32_t rs, const uint32_t (&hb)[n_words(R, WSH)],
                                                      const SINK &sink) {
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int j = fold_bin_generic(p.x, p.y, invP[SHARE_P ? 0 : r], cc[r], n_phi);
-        sink((uint32_t)j * rs + hb[r >> 1], r);
+        sink((uint32_t)j * rs + hb[r >> WSH], r);
     }
 }
-template <int R, bool SHARE_P, typename SINK>
+template <int R, bool SHARE_P, int WSH = 1, typename SINK>
 __device__ __forceinline__ void fold_range_generic(const double2 *__restrict__ sp, int kk, const int ke,
                                                    const double (&invP)[R], const double (&cc)[R], const int n_phi,
-                                                   const uint32_t rs, const uint32_t (&hb)[(R + 1) / 2], const SINK &sink) {
-    for (; kk < ke; ++kk) fold_bin_add_generic<R, SHARE_P>(sp[kk], invP, cc, n_phi, rs, hb, sink);
+                                                   const uint32_t rs, const uint32_t (&hb)[n_words(R, WSH)], const SINK &sink) {
+    for (; kk < ke; ++kk) fold_bin_add_generic<R, SHARE_P, WSH>(sp[kk], invP, cc, n_phi, rs, hb, sink);
 }
 
 // S4, first half: close magnitude bin `seg_i`.  fetch_word reads and clears this thread's counter word of phase bin j
@@ -170,19 +178,27 @@ __device__ __forceinline__ uint32_t fetch_word(const int j, const int n_phi, con
 
 // DUMP (gce_ce_debug_histogram): dpos[r] is the position of slot r's trial in the caller's list (-1: not listed); the
 // count this word contributes to Eq. 4 is written to out_counts[lc][dpos][j][seg_i].
-template <int R, bool DUMP, bool BIG>
+template <int R, bool DUMP, bool BIG, bool WIDE>
 __device__ __forceinline__ void close_word(const uint32_t w, const int j, const int w2, const int n_phi, const uint32_t us,
                                            int64_t (&S2)[R], const int64_t *__restrict__ sL, const SearchParams &prm,
                                            const int lc, const int (&dpos)[R], const int seg_i) {
-    int64_t v0, v1;
-    ltab_pair<BIG>(sL, prm.ltab, w, us, v0, v1);
-    S2[2 * w2] += v0;
-    if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
-    if (DUMP) {
-        const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
-        const int d0 = dpos[2 * w2], d1 = dpos[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0];
-        if (d0 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d0) * n_phi + j) * prm.n_m + seg_i] = c0;
-        if (2 * w2 + 1 < R && d1 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d1) * n_phi + j) * prm.n_m + seg_i] = c1;
+    if constexpr (WIDE) {  // word w2 is the 32-bit count of trial slot w2
+        S2[w2 < R ? w2 : 0] += ltab_one(sL, prm.ltab, w);
+        if (DUMP) {
+            const int d0 = dpos[w2 < R ? w2 : 0];
+            if (d0 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d0) * n_phi + j) * prm.n_m + seg_i] = w;
+        }
+    } else {
+        int64_t v0, v1;
+        ltab_pair<BIG>(sL, prm.ltab, w, us, v0, v1);
+        S2[(2 * w2) < R ? 2 * w2 : 0] += v0;
+        if (2 * w2 + 1 < R) S2[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
+        if (DUMP) {
+            const uint32_t c0 = (w & 0xffffu) >> us, c1 = w >> (16u + us);
+            const int d0 = dpos[(2 * w2) < R ? 2 * w2 : 0], d1 = dpos[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0];
+            if (d0 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d0) * n_phi + j) * prm.n_m + seg_i] = c0;
+            if (2 * w2 + 1 < R && d1 >= 0) prm.out_counts[(((int64_t)lc * prm.n_dump + d1) * n_phi + j) * prm.n_m + seg_i] = c1;
+        }
     }
 }
 
@@ -193,13 +209,13 @@ __device__ __forceinline__ void close_word(const uint32_t w, const int j, const 
 // OVL (NEXT item N2): 50 %-overlapping phase bins -- bin k holds the plain cells k-1 and k (cyclic), so
 // the looked-up count is w[k] + w[k-1] (packed 16-bit pairs; needs 2N <= 65535); the folds and the plain marginal are
 // unchanged, the overlap costs one add per word.
-template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL, bool EXT>
+template <int NPHI, bool REGM, int R, bool DUMP, bool BIG, bool OVL, bool EXT, bool WIDE>
 __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs, const uint32_t marg_off, const uint32_t us,
-                                              const uint32_t (&hb)[(R + 1) / 2],
-                                              uint32_t (&mg)[REGM ? NPHI : 1][(R + 1) / 2], int64_t (&S2)[R],
+                                              const uint32_t (&hb)[n_words(R, WIDE ? 0 : 1)],
+                                              uint32_t (&mg)[REGM ? NPHI : 1][n_words(R, WIDE ? 0 : 1)], int64_t (&S2)[R],
                                               const int64_t *__restrict__ sL, const SearchParams &prm, const int lc,
                                               const int (&dpos)[R], const int seg_i) {
-    constexpr int RW = (R + 1) / 2;
+    constexpr int RW = n_words(R, WIDE ? 0 : 1);
     uint32_t prev[RW], first[RW];
     if (NPHI > 0) {
         constexpr int NP = NPHI > 0 ? NPHI : 1;
@@ -218,10 +234,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
                     const uint32_t ww = w[jj][w2];
                     if (REGM) mg[REGM ? j0 + jj : 0][w2] += ww;
                     else red_add_u32(hb[w2] + marg_off + (uint32_t)(j0 + jj - w2) * rs, ww);
-                    if (!OVL) close_word<R, DUMP, BIG>(ww, j0 + jj, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
+                    if (!OVL) close_word<R, DUMP, BIG, WIDE>(ww, j0 + jj, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                     else {
                         if (j0 + jj == 0) first[w2] = ww;
-                        else close_word<R, DUMP, BIG>(ww + prev[w2], j0 + jj, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
+                        else close_word<R, DUMP, BIG, WIDE>(ww + prev[w2], j0 + jj, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                         prev[w2] = ww;
                     }
                 }
@@ -232,10 +248,10 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
             for (int w2 = 0; w2 < RW; ++w2) {
                 const uint32_t ww = fetch_word<EXT>(j, n_phi, rs, hb[w2]);
                 red_add_u32(hb[w2] + marg_off + (uint32_t)(j - w2) * rs, ww);
-                if (!OVL) close_word<R, DUMP, BIG>(ww, j, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
+                if (!OVL) close_word<R, DUMP, BIG, WIDE>(ww, j, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                 else {
                     if (j == 0) first[w2] = ww;
-                    else close_word<R, DUMP, BIG>(ww + prev[w2], j, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
+                    else close_word<R, DUMP, BIG, WIDE>(ww + prev[w2], j, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
                     prev[w2] = ww;
                 }
             }
@@ -244,7 +260,7 @@ __device__ __forceinline__ void close_mag_bin(const int n_phi, const uint32_t rs
     if (OVL) {  // bin 0 = cells n_phi-1 and 0
 #pragma unroll
         for (int w2 = 0; w2 < RW; ++w2)
-            close_word<R, DUMP, BIG>(first[w2] + prev[w2], 0, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
+            close_word<R, DUMP, BIG, WIDE>(first[w2] + prev[w2], 0, w2, n_phi, us, S2, sL, prm, lc, dpos, seg_i);
     }
 }
 
@@ -303,11 +319,16 @@ __device__ __forceinline__ void sort_slots_by_c(double (&cc)[R], int64_t (&qv)[R
 // thread share one period (n_pdot % R == 0).  EXT: 2 n_phi + 1 counter rows, shared floors (fold_bin_add MODE 1 / 2).
 // DUMP (gce_ce_debug_histogram): the same kernel, plan and tiles as the search, but only tiles that hold a listed trial
 // are processed and, instead of the search outputs, the count tables (and CE) of the listed trials are written.
-template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT, int NTC>
+// WIDE (NEXT item N3, "light curves of any length"): one 32-bit counter per trial instead of two 16-bit
+// fields per word, for calls whose light curves may exceed the 16-bit range (gce_ce_params.max_lc_points); counts are
+// looked up directly (no byte-offset trick), the k ln k table is as long as the longest light curve.
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT, int NTC, bool WIDE = false>
 __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchParams prm) {
     static_assert(!REGM || NPHI > 0, "register marginals need a compile-time n_phi");
-    static_assert(!EXT || (SHARE_P && R % 2 == 0), "extended rows serve trial pairs that share a period");
-    constexpr int RW = (R + 1) / 2;  // 32-bit words per (bin, thread): two 16-bit counters each
+    static_assert(!EXT || (SHARE_P && R % 2 == 0 && !WIDE), "extended rows serve trial pairs that share a period");
+    static_assert(!WIDE || !REGM, "wide counters: generic family only");
+    constexpr int WSH = WIDE ? 0 : 1;
+    constexpr int RW = n_words(R, WSH);  // 32-bit words per (bin, thread): two 16-bit counters each, or one 32-bit counter
     constexpr int NPHI_REG = REGM ? NPHI : 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int NT = NTC > 0 ? NTC : (int)blockDim.x, NW = NT >> 5;
@@ -382,9 +403,9 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
 #pragma unroll
     for (int w2 = 0; w2 < RW; ++w2) hb[w2] = smem_u32(hist) + (uint32_t)tid * 4u + (uint32_t)w2 * plane;
     const bool ovl = prm.overlap != 0;  // N2: 2N table entries per trial
-    const double ce_scale = N > 0 ? ldexp(1.0, -kLfixShift) / (double)(ovl ? 2 * N : N) : 0.0;
-    const uint32_t us = ((ovl ? 2 : 1) * N <= 8191) ? 3u : 0u;  // counter unit 2^us: a field is its table entry's byte offset
-    const RedSink sink{1u << us, 0x10000u << us};
+    const double ce_scale = N > 0 ? ldexp(1.0, -prm.info[lc].lshift) / (double)(ovl ? 2 * N : N) : 0.0;
+    const uint32_t us = (!WIDE && (ovl ? 2 : 1) * N <= 8191) ? 3u : 0u;  // counter unit 2^us: a field is its table entry's byte offset
+    const RedSink sink{1u << us, WIDE ? 1u : 0x10000u << us};
     uint32_t mg[NPHI_REG][RW];  // phase marginal n_j of the R trials (NPHI > 0), packed like the histogram
 #pragma unroll
     for (int j = 0; j < NPHI_REG; ++j)
@@ -468,28 +489,31 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                 // ---------------- hot loop: fold + bin the points of magnitude bin seg_i that are in this buffer
                 if (lo < hi) {
                     if (fast) {
-                        if (pz) fold_range<R, SHARE_P, true, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
-                        else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
-                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
-                        else fold_range<R, SHARE_P, false, 0>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        if (pz) fold_range<R, SHARE_P, true, 0, WSH>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        else if (EXT && quad_ok) fold_range<R, SHARE_P, false, EXT ? 2 : 0, WSH>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        else if (EXT && pair_ok) fold_range<R, SHARE_P, false, EXT ? 1 : 0, WSH>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
+                        else fold_range<R, SHARE_P, false, 0, WSH>(sp, lo, hi, invP, cc, nphi_d, negn, rs, hb, sink);
                     } else {
-                        fold_range_generic<R, SHARE_P>(sp, lo, hi, invP, cc, n_phi, rs, hb, sink);
+                        fold_range_generic<R, SHARE_P, WSH>(sp, lo, hi, invP, cc, n_phi, rs, hb, sink);
                     }
                 }
                 if (b1 > k_end) break;  // the bin continues in the next buffer
                 // ---------------- S4: the bin is complete; a cell holds at most b1 - b0 points
                 if (b1 > b0) {
                     // a cell of this bin holds at most b1 - b0 points (twice that with overlapping bins)
-                    if (!ovl) {
+                    if constexpr (WIDE) {
+                        if (!ovl) close_mag_bin<NPHI, REGM, R, DUMP, true, false, EXT, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                        else close_mag_bin<NPHI, REGM, R, DUMP, true, true, EXT, true>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                    } else if (!ovl) {
                         if (us == 3u && b1 - b0 < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, DUMP, false, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, false, EXT, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, DUMP, true, false, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, false, EXT, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                     } else {
                         if (us == 3u && 2 * (b1 - b0) < kLtabSmem)
-                            close_mag_bin<NPHI, REGM, R, DUMP, false, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, false, true, EXT, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                         else
-                            close_mag_bin<NPHI, REGM, R, DUMP, true, true, EXT>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
+                            close_mag_bin<NPHI, REGM, R, DUMP, true, true, EXT, false>(n_phi, rs, marg_off, us, hb, mg, S2, sL, prm, lc, dpos, seg_i);
                     }
                 }
                 ++seg_s;
@@ -507,10 +531,14 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
         for (int r = 0; r < R; ++r) S1[r] = 0;
         if (N > 0) {
             auto add_marg = [&](const uint32_t w, const int w2, auto big) {
-                int64_t v0, v1;
-                ltab_pair<decltype(big)::value>(sL, prm.ltab, w, us, v0, v1);
-                S1[2 * w2] += v0;
-                if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
+                if constexpr (WIDE) {
+                    S1[w2 < R ? w2 : 0] += ltab_one(sL, prm.ltab, w);
+                } else {
+                    int64_t v0, v1;
+                    ltab_pair<decltype(big)::value>(sL, prm.ltab, w, us, v0, v1);
+                    S1[(2 * w2) < R ? 2 * w2 : 0] += v0;
+                    if (2 * w2 + 1 < R) S1[(2 * w2 + 1) < R ? 2 * w2 + 1 : 0] += v1;
+                }
             };
             auto marg_pass = [&](auto big, auto ovlt) {
                 constexpr bool OVL = decltype(ovlt)::value;
@@ -657,9 +685,9 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
 }
 
 // Host side of one instantiation: opt in to the dynamic shared memory once per device, then launch.
-template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT, int NTC>
+template <int NPHI, bool REGM, int R, bool SHARE_P, bool DUMP, bool EXT, int NTC, bool WIDE = false>
 cudaError_t launch_search(const SearchParams &sp, const Plan &plan, int32_t n_lc, cudaStream_t st) {
-    auto kern = k_search<NPHI, REGM, R, SHARE_P, DUMP, EXT, NTC>;
+    auto kern = k_search<NPHI, REGM, R, SHARE_P, DUMP, EXT, NTC, WIDE>;
     static std::mutex mu;
     static size_t smem_set[64] = {};  // largest opt-in made so far, per device
     int dev = 0;

@@ -22,8 +22,15 @@ cudaError_t GCE_LAUNCHER_NAME(GCE_FAMILY, GCE_DUMP)(const SearchParams &sp, cons
     constexpr bool D = GCE_DUMP != 0;
     constexpr int N = GCE_FAMILY;
     if (plan.nphi_t != N) return cudaErrorInvalidValue;
+    if (plan.wide && N != 0) return cudaErrorInvalidValue;
 #if GCE_FAMILY == 0
     if (plan.regm || plan.ext) return cudaErrorInvalidValue;
+    if (plan.wide) {  // 32-bit counters (N3: light curves of any length)
+        if (plan.share_p && plan.R == 4) return launch_search<0, false, 4, true, D, false, 0, true>(sp, plan, n_lc, st);
+        if (plan.share_p && plan.R == 2) return launch_search<0, false, 2, true, D, false, 0, true>(sp, plan, n_lc, st);
+        if (!plan.share_p && plan.R == 4) return launch_search<0, false, 4, false, D, false, 0, true>(sp, plan, n_lc, st);
+        return cudaErrorInvalidValue;
+    }
     if (plan.share_p && plan.R == 4) return launch_search<0, false, 4, true, D, false, 0>(sp, plan, n_lc, st);
     if (plan.share_p && plan.R == 2) return launch_search<0, false, 2, true, D, false, 0>(sp, plan, n_lc, st);
     if (!plan.share_p && plan.R == 4) return launch_search<0, false, 4, false, D, false, 0>(sp, plan, n_lc, st);

@@ -9,7 +9,8 @@ namespace {
 // base[lc * lc_stride + p * part_stride + ...], p < n_parts: inside one call the parts are the CTAs (jobs) of k_search,
 // in gce_ce_merge_partials they are the caller's partial blobs (period ranges, batches, GPUs).  Keys are
 // the exact integers (S = N*CE*2^42, flat q), so the merged result does not depend on the split.
-// Partial blob of one light curve (int64 words): [0,K) S ascending, [K,2K) q, [2K,2K+8) Eq. 5 sums, [2K+8] N, [2K+9] pivot.
+// Partial blob of one light curve (int64 words): [0,K) S ascending, [K,2K) q, [2K,2K+8) Eq. 5 sums,
+// [2K+8] N in the low 32 bits and the table's fixed-point shift above them, [2K+9] pivot.
 __host__ __device__ inline int partial_words(int K) { return 2 * K + kStatWords + 2; }
 
 __global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ S, const int64_t *__restrict__ q,
@@ -34,9 +35,11 @@ __global__ void __launch_bounds__(32) k_merge_topk(const int64_t *__restrict__ S
         return;
     }
     const bool have = top.S != kInfS;
-    const int64_t n = info ? (int64_t)info[lc].n : npts[(int64_t)lc * npts_stride];
+    const int64_t nw = info ? (int64_t)info[lc].n | ((int64_t)info[lc].lshift << 32) : npts[(int64_t)lc * npts_stride];
+    const int64_t n = nw & 0xffffffffll;
+    const int lshift = (int)(nw >> 32);
     out_idx[(int64_t)lc * K + lane] = have ? top.q : -1;
-    if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -kLfixShift) / (double)(mult * n))) : CUDART_NAN_F;
+    if (out_ce) out_ce[(int64_t)lc * K + lane] = have ? (float)((double)top.S * (ldexp(1.0, -lshift) / (double)(mult * n))) : CUDART_NAN_F;
 }
 
 // Eq. 5: sums the partials (exact integers) and converts once to fp64:
@@ -58,12 +61,14 @@ __global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__
     __syncwarp();
     if (lane != 0) return;
     for (int l = 1; l < 32; ++l) stat_merge(acc, sh[l]);
-    const int64_t n_pts = info ? (int64_t)info[lc].n : npts[(int64_t)lc * npts_stride];
+    const int64_t nw = info ? (int64_t)info[lc].n | ((int64_t)info[lc].lshift << 32) : npts[(int64_t)lc * npts_stride];
+    const int64_t n_pts = nw & 0xffffffffll;
+    const int lshift = (int)(nw >> 32);
     const int64_t pivot = info ? info[lc].K : npts[(int64_t)lc * npts_stride + 1];
     if (out_raw) {
         int64_t *o = out_raw + (int64_t)lc * raw_stride;
         for (int i = 0; i < kStatWords; ++i) o[i] = (int64_t)acc[i];
-        o[kStatWords] = n_pts;
+        o[kStatWords] = nw;
         o[kStatWords + 1] = pivot;
         return;
     }
@@ -74,7 +79,7 @@ __global__ void __launch_bounds__(32) k_merge_stats(const uint64_t *__restrict__
     const bool neg = (acc[2] >> 63) != 0;
     const double sum_d = neg ? -u128_to_double((u128_t)0 - A) : u128_to_double(A);
     const double sum_d2 = (double)acc[5] * 3.4028236692093846e38 + u128_to_double(((u128_t)acc[4] << 64) | acc[3]);
-    const double scale = ldexp(1.0, -kLfixShift) / (double)(mult * n_pts);
+    const double scale = ldexp(1.0, -lshift) / (double)(mult * n_pts);
     const double mean_d = sum_d / n;
     double var = sum_d2 / n - mean_d * mean_d;
     if (var < 0.0 || acc[6] == acc[7]) var = 0.0;  // min == max: every trial has the same CE, the spread is exactly 0

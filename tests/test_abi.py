@@ -73,10 +73,14 @@ def test_validate_host(gce):
     m2 = m.copy()
     m2[3] = np.nan
     assert gce.gce_ce_validate_host(t, m2, [0, 4, 10], [100.0], [0.0], prm) == -2
-    # length limits: 65535 points per light curve, 32767 with overlapping bins (2N table entries, 16-bit pairs)
+    # lengths beyond the 16-bit counter range (65535 points, 32767 with overlapping bins) are accepted by the host
+    # entries (they switch to 32-bit counters themselves); the limit is GCE_CE_MAX_POINTS_WIDE
     big = np.zeros(40000)
     assert gce.gce_ce_validate_host(big, big, [0, 40000], [100.0], [0.0], prm) == 0
-    assert gce.gce_ce_validate_host(big, big, [0, 40000], [100.0], [0.0], gce.make_params(20, 10, overlap=True)) == -2
+    assert gce.gce_ce_validate_host(big, big, [0, 40000], [100.0], [0.0], gce.make_params(20, 10, overlap=True)) == 0
+    # params out of range
+    assert gce.gce_ce_validate_host(t, m, [0, 4, 10], [100.0], [0.0], gce.make_params(20, 10, max_lc_points=(1 << 26) + 1)) == -2
+    assert gce.gce_ce_validate_host(t, m, [0, 4, 10], [100.0], [0.0], gce.make_params(20, 10, max_lc_points=-1)) == -2
 
 
 def test_product_does_not_import_the_oracle():

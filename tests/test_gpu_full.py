@@ -250,6 +250,92 @@ def test_long_light_curves_are_streamed(gce, oracle, n_obs, n_phi, n_m, n_pdot):
     assert np.array_equal(counts[0].cpu().numpy().astype(np.int64), refc)
 
 
+def _long_batch(n_obs, seed):
+    rng = np.random.default_rng(seed)
+    t_long = np.sort(rng.uniform(0, 3e7, n_obs))
+    m_long = W.two_dip_mags(rng, t_long, 611.0, -2e-11, 0.5, 0.2, 0.05)
+    t_short = np.sort(rng.uniform(0, 3e7, 300))
+    m_short = rng.normal(size=300)
+    return (np.concatenate([t_long, t_short]), np.concatenate([m_long, m_short]),
+            np.array([0, n_obs, n_obs + 300], dtype=np.int64), t_long, m_long)
+
+
+@pytest.mark.parametrize("n_obs,n_phi,n_m,n_pdot,overlap", [(100000, 20, 10, 4, False), (70001, 30, 7, 2, False),
+                                                            (100000, 50, 10, 2, True), (40000, 15, 10, 1, True)])
+def test_light_curves_beyond_the_16_bit_counters(gce, oracle, n_obs, n_phi, n_m, n_pdot, overlap):
+    """NEXT item N3 (light curves of any length): a call that announces light curves longer than 65 535
+    points (32 767 with overlapping bins) runs with 32-bit counters and a k ln k table as long as the light curve
+    (whose fixed-point shift drops below 42 once it has more than 2^17 entries).  Cube, selection, Eq. 5 and bit-exact
+    counts against the oracle, next to a short light curve in the same batch."""
+    times, mags, offs, t_long, m_long = _long_batch(n_obs, n_obs + n_phi)
+    periods = 1.0 / np.linspace(1 / 900.0, 1 / 300.0, 300)
+    pdots = np.linspace(-4e-11, 0.0, n_pdot) if n_pdot > 1 else np.zeros(1)
+    ref = oracle.ce_search(times, mags, offs, periods, pdots, n_phi, n_m, overlap=overlap)
+    res = gce.search(dev(times), dev(mags), dev(offs), dev(periods), dev(pdots), n_phi, n_m, top_k=4, want_cube=True,
+                     ce_fp64=True, want_stats=True, overlap=overlap)
+    torch.cuda.synchronize()
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    for lc in range(2):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 4, RTOL64, oracle)
+        mu, sigma, rho = oracle.significance(ref[lc])
+        st = res.stats[lc].cpu().numpy()
+        np.testing.assert_allclose(st[:3], [mu, sigma, ref[lc].min()], rtol=1e-9)
+    # bit-exact counts of a few trials of the long light curve, from the kernel the search ran (with overlap = 1 the
+    # dump holds the overlapped table the entropy is taken from)
+    q = torch.tensor([0, 1, 299 * n_pdot + n_pdot - 1], dtype=torch.int64, device="cuda")
+    prm = gce.make_params(n_phi, n_m, overlap=overlap, max_lc_points=n_obs)
+    counts = torch.empty((2, 3, n_phi, n_m), dtype=torch.int32, device="cuda")
+    ws = torch.empty(gce.gce_ce_workspace_bytes(times.size, 2, 300, n_pdot, prm), dtype=torch.uint8, device="cuda")
+    gce.gce_ce_debug_histogram(dev(times), dev(mags), dev(offs), dev(periods), dev(pdots), prm, q, counts, None, ws)
+    torch.cuda.synchronize()
+    refc = oracle.histogram(t_long, m_long, periods, pdots, n_phi, n_m, q.cpu().numpy())
+    if overlap:
+        refc = np.stack([oracle.overlap_counts(r) for r in refc])
+    assert np.array_equal(counts[0].cpu().numpy().astype(np.int64), refc)
+    # the host entry sees the lengths and switches to the 32-bit counters itself: same bits
+    ce_h = np.empty((2, 300, n_pdot), dtype=np.float64)
+    idx_h = np.empty((2, 4), dtype=np.int64)
+    gce.gce_ce_search_host(times, mags, offs, periods, pdots, gce.make_params(n_phi, n_m, top_k=4, ce_fp64=True, overlap=overlap),
+                           ce_h, idx_h, None)
+    assert np.array_equal(ce_h, res.ce.cpu().numpy()) and np.array_equal(idx_h, res.best_idx.cpu().numpy())
+
+
+def test_unannounced_long_light_curve_is_treated_as_empty(gce):
+    """Device-pointer call without max_lc_points: the lengths live on the device, so a light curve beyond the 16-bit
+    range cannot be refused up front; it is never folded with wrapped counters but treated as empty (NaN, -1), and the
+    other light curves of the batch are unaffected.  When total_points alone proves it the call is refused."""
+    times, mags, offs, _, _ = _long_batch(70000, 5)
+    periods = 1.0 / np.linspace(1 / 900.0, 1 / 300.0, 64)
+    pdots = np.zeros(1)
+    prm = gce.make_params(20, 10, top_k=2)
+    ce = torch.empty((2, 64, 1), dtype=torch.float32, device="cuda")
+    idx = torch.empty((2, 2), dtype=torch.int64, device="cuda")
+    ws = torch.empty(gce.gce_ce_workspace_bytes(times.size, 2, 64, 1, prm), dtype=torch.uint8, device="cuda")
+    gce.gce_ce_search(dev(times), dev(mags), dev(offs), dev(periods), dev(pdots), prm, ce, idx, None, None, ws)
+    torch.cuda.synchronize()
+    assert torch.isnan(ce[0]).all() and (idx[0] == -1).all()
+    assert torch.isfinite(ce[1]).all() and (idx[1] >= 0).all()
+    one = np.array([0, 70000], dtype=np.int64)
+    with pytest.raises(gce.GceError) as e:
+        gce.gce_ce_search(dev(times[:70000]), dev(mags[:70000]), dev(one), dev(periods), dev(pdots), prm, ce[:1], idx[:1], None, None, ws)
+    assert e.value.code == -2
+
+
+def test_wide_counters_period_split_is_exact(gce):
+    """The partial blob carries the table's fixed-point shift, so a period-split search of a long light curve merges to
+    the bits of the unsplit call."""
+    times, mags, offs, _, _ = _long_batch(140000, 6)
+    periods = 1.0 / np.linspace(1 / 900.0, 1 / 300.0, 96)
+    pdots = np.linspace(-4e-11, 0.0, 2)
+    args = (dev(times), dev(mags), dev(offs), dev(periods), dev(pdots), 20, 10)
+    whole = gce.search(*args, top_k=3, want_cube=False, want_stats=True)
+    # search_period_chunks builds its own params: announce the length through the keyword
+    split = gce.search_period_chunks(*args, [(0, 40), (40, 41), (41, 96)], top_k=3, want_stats=True, max_lc_points=140000)
+    torch.cuda.synchronize()
+    assert torch.equal(whole.best_idx, split.best_idx) and torch.equal(whole.best_ce, split.best_ce)
+    assert torch.equal(whole.stats, split.stats)
+
+
 # ------------------------------------------------------------------------------------------ N1: fused Eq. 5 statistics
 RTOL_STATS = 1e-9   # DESIGN.md section 10: exact integer sums of N*CE*2^42, one fp64 conversion; the per-trial CE values
                     # differ from the oracle's by <= 1e-12 relative, the variance subtraction amplifies that by mean^2/var

@@ -2,9 +2,12 @@
 
 gce_ce_search_partial over disjoint period ranges + gce_ce_merge_partials must reproduce gce_ce_search on the whole grid
 bit for bit (indices, fp32 CE, Eq. 5 statistics), however the grid is split, because every key and sum is an integer.
-The two-"rank" case runs the ranks one after the other on the one GPU (they do not wait on each other) and merges
-their blobs as the all-gather of bench / search_period_chunks would deliver them.
+One two-"rank" case runs the ranks one after the other in one process and concatenates their blobs; the other runs
+search_period_chunks(dist=...) in two real processes (world_size 2, gloo all-gather of the host-staged blobs, both ranks
+on cuda:0 -- their kernels never wait on one another).
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -48,7 +51,10 @@ def test_period_chunks_merge_bit_exactly(gce, name, kw, k, overlap):
         assert torch.equal(res.best_ce, whole.best_ce), cuts
         assert np.array_equal(res.stats.cpu().numpy(), whole.stats.cpu().numpy()), cuts
         for (a, b) in chunks:
-            assert torch.equal(slices[(a, b)], whole.ce[:, a:b, :]), (cuts, a)
+            if b > a:   # the sink is called for non-empty slices only
+                assert torch.equal(slices[(a, b)], whole.ce[:, a:b, :]), (cuts, a)
+            else:
+                assert (a, b) not in slices
 
 
 def test_two_ranks_split_the_period_axis(gce):
@@ -121,3 +127,47 @@ def test_host_entry_pipelines_large_cubes_bit_exactly(gce):
     ce2 = np.zeros_like(ce)
     gce.gce_ce_search_host(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, prm0, ce2, None, None, None)
     assert np.array_equal(ce2, ce)
+
+
+def _period_split_rank(rank, world, port, result_dir):
+    """One real process per rank (both on cuda:0; the exchange is gloo's all_gather of the host-staged blobs: NCCL
+    refuses two ranks on one GPU).  The ranks' kernels never wait on one another: each rank searches its own period
+    ranges, the only exchange is the all-gather of n_lc x (2k + 10) int64 blobs, after which every rank merges."""
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import paper_2006_06866_b200 as gce
+        torch.cuda.set_device(0)
+        w = W.make("C3", n_lc=1, n_p=3000, n_pdot=32)     # one deep target: fewer light curves than ranks
+        args = (d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), 20, 10)
+        chunks = [[(0, 700), (700, 1400)], [(1400, 3000)]][rank]   # complementary halves, unequal chunk counts
+        side = torch.cuda.Stream()
+        got = gce.search_period_chunks(*args, chunks, top_k=5, want_stats=True, dist=dist, stream=side)
+        whole = gce.search(*args, top_k=5, want_cube=False, want_stats=True)
+        torch.cuda.synchronize()
+        ok = (torch.equal(got.best_idx, whole.best_idx) and torch.equal(got.best_ce, whole.best_ce)
+              and np.array_equal(got.stats.cpu().numpy(), whole.stats.cpu().numpy()))
+        # a rank with no periods at all still takes part in the exchange
+        chunks2 = [[(0, 3000)], []][rank]
+        got2 = gce.search_period_chunks(*args, chunks2, top_k=5, want_stats=True, dist=dist)
+        torch.cuda.synchronize()
+        ok = ok and torch.equal(got2.best_idx, whole.best_idx) and np.array_equal(got2.stats.cpu().numpy(), whole.stats.cpu().numpy())
+        with open(os.path.join(result_dir, f"rank{rank}.txt"), "w") as f:
+            f.write("ok" if ok else "mismatch")
+    finally:
+        dist.destroy_process_group()
+
+
+def test_period_axis_split_in_two_processes(gce, tmp_path):
+    """SURVEY.md 8(e) / PAPER.md:234: the period-axis split with its one collective, run in two real processes
+    (world_size 2): every rank's selection and Eq. 5 statistics are bit-equal to the unsplit call."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_period_split_rank, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    for r in range(2):
+        assert (tmp_path / f"rank{r}.txt").read_text() == "ok"
