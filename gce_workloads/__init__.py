@@ -268,6 +268,29 @@ def make(name: str, **kw) -> Workload:
     return CONFIGS[name.upper()](**kw)
 
 
+def two_filter_batch(seed, n_lc=4, n_obs=400, n_p=600, n_pdot=4, offset=0.9, scale=0.6):
+    """N4: light curves observed in two filters merged into one time series.  Filter 1 sees the same
+    two-dip signal `offset` mag fainter with its dips scaled by `scale` (a colour term) and its own noise; about 40 % of
+    the points are in filter 1.  Returns (Workload, filter_ids int32[sum N])."""
+    rng = np.random.default_rng(seed)
+    lcs, filt, truth_p = [], [], []
+    for _ in range(n_lc):
+        t = np.sort(rng.uniform(0.0, 2.0 * 365.25 * DAY, size=n_obs))
+        P = float(np.exp(rng.uniform(np.log(400.0), np.log(2000.0))))
+        f = (rng.uniform(size=n_obs) < 0.4).astype(np.int32)
+        clean = two_dip_mags(rng, t, P, 0.0, 0.5, 0.25, 0.0)
+        m = np.where(f == 0, clean, 18.0 + offset + scale * (clean - 18.0))
+        m = m + rng.normal(0.0, np.where(f == 0, 0.03, 0.05))
+        lcs.append((t, m))
+        filt.append(f)
+        truth_p.append(P)
+    times, mags, offs = _pack(lcs)
+    w = Workload(f"twofilter{seed}", times, mags, offs, _freq_grid(1 / 2400.0, 1 / 350.0, n_p),
+                 np.ascontiguousarray(np.linspace(-2e-11, 0.0, int(n_pdot))) if n_pdot > 1 else np.zeros(1), 20, 10, 3, True,
+                 truth={"P": np.array(truth_p)})
+    return w, np.ascontiguousarray(np.concatenate(filt), dtype=np.int32)
+
+
 # ----------------------------------------------------------------------------- small helpers for tests
 def random_batch(seed, n_lc, n_min, n_max, n_p, n_pdot, n_phase_bins=20, n_mag_bins=10, top_k=3,
                  pdot_range=(-1e-9, 1e-10), baseline_days=400.0) -> Workload:

@@ -66,6 +66,7 @@ def lib():
         L.gce_oracle_ce_search_overlap.argtypes = L.gce_oracle_ce_search.argtypes
         L.gce_oracle_ce_at_overlap.argtypes = L.gce_oracle_ce_at.argtypes
         L.gce_oracle_overlap_counts.argtypes = [_i64p, C.c_int32, C.c_int32, _i64p]
+        L.gce_oracle_normalise_filters.argtypes = [_f64p, _i32p, C.c_int64, _f64p]
         L.gce_oracle_topk.argtypes = [_f64p, C.c_int64, C.c_int32, _i64p, _f64p]
         L.gce_oracle_significance.argtypes = [_f64p, C.c_int64, _f64p]
         L.gce_oracle_num_threads.restype = C.c_int
@@ -90,6 +91,26 @@ def preprocess(times, mags, n_mag_bins):
     _check(lib().gce_oracle_preprocess(_p(t, _f64p), _p(m, _f64p), n, int(n_mag_bins),
                                        _p(dt, _f64p), _p(dt2, _f64p), _p(mbin, _i32p)))
     return dt, dt2, mbin
+
+
+def normalise(mags, filter_ids=None):
+    """S0 (N4) for ONE light curve: per-filter (median, population std) normalisation -> u[N]."""
+    m = _f64(mags)
+    n = m.shape[0]
+    u = np.empty(n)
+    f = None if filter_ids is None else np.ascontiguousarray(filter_ids, dtype=np.int32)
+    _check(lib().gce_oracle_normalise_filters(_p(m, _f64p), None if f is None else _p(f, _i32p), n, _p(u, _f64p)))
+    return u
+
+
+def normalise_batch(mags, lc_offsets, filter_ids=None):
+    """S0 applied light curve by light curve to a CSR batch -> the magnitudes the search then bins."""
+    m, offs = _f64(mags), _i64(lc_offsets)
+    out = np.empty_like(m)
+    for l in range(offs.shape[0] - 1):
+        a, b = int(offs[l]), int(offs[l + 1])
+        out[a:b] = normalise(m[a:b], None if filter_ids is None else np.asarray(filter_ids)[a:b])
+    return out
 
 
 def fold_bins(dt, dt2, P, Pdot, n_phase_bins):

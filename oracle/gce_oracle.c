@@ -7,7 +7,8 @@
  * includes the other.  Host pointers only; plain C; fp64 throughout.
  *
  * Written from /root/reference/PAPER.md (Katz et al., arXiv 2006.06866):
- *   - magnitude normalisation            PAPER.md:96   (reading Q2 of DESIGN.md: min/max -> [0,1])
+ *   - magnitude normalisation            PAPER.md:96   (reading Q2 of DESIGN.md: min/max -> [0,1]; the paper's own
+ *                                                       per-filter median / std step as an option, reading Q19)
  *   - phase fold with Pdot, Eq. 3
  *   - 2-D phase x magnitude histogram     PAPER.md:106  (non-overlapping bins; the 50 %-overlapping variant: reading Q3)
  *   - conditional entropy, Eq. 4
@@ -44,6 +45,58 @@
 
 #define GCE_ORACLE_OK 0
 #define GCE_ORACLE_EINVAL -1
+
+/* ---------------------------------------------------------------------------------------
+ * S0 (optional, NEXT item N4)  the paper's normalisation: "subtract from each
+ * observation the median magnitude value, and then we divide by the standard deviation of the
+ * magnitude values ... this allows us to combine observations from different filters into one
+ * input light curve".  Per filter f of one light curve, over the points k with filt[k] == f in
+ * light-curve order (reading Q19):
+ *     med  = median (middle value, or the mean of the two middle values: (a + b) * 0.5)
+ *     mean = (((v_0 + v_1) + v_2) + ...) / n_f              sequential sum, RN
+ *     sd   = sqrt( (((d_0^2 + d_1^2) + ...) / n_f) ),  d_k = v_k - mean   population (ddof 0)
+ *     u_k  = (v_k - med) / sd ;  sd == 0 (one point, or all equal) -> u_k = 0
+ * The merged u then goes through S1 (min/max bins over the merged range) unchanged.
+ * filt == NULL: one filter.  Filter ids 0 .. 7.
+ * ------------------------------------------------------------------------------------- */
+static int cmp_double(const void *a, const void *b)
+{
+    const double x = *(const double *)a, y = *(const double *)b;
+    return (x > y) - (x < y);
+}
+
+int gce_oracle_normalise_filters(const double *m, const int32_t *filt, int64_t n, double *u)
+{
+    if (n < 0) return GCE_ORACLE_EINVAL;
+    double *v = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    if (!v) return GCE_ORACLE_EINVAL;
+    for (int32_t f = 0; f < 8; ++f) {
+        int64_t nf = 0;
+        for (int64_t k = 0; k < n; ++k) {
+            const int32_t fk = filt ? filt[k] : 0;
+            if (fk < 0 || fk > 7) { free(v); return GCE_ORACLE_EINVAL; }
+            if (fk == f) v[nf++] = m[k];
+        }
+        if (nf == 0) continue;
+        double sum = 0.0;
+        for (int64_t i = 0; i < nf; ++i) sum = sum + v[i];
+        const double mean = sum / (double)nf;
+        double ss = 0.0;
+        for (int64_t i = 0; i < nf; ++i) {
+            const double d = v[i] - mean;
+            ss = ss + d * d;
+        }
+        const double sd = sqrt(ss / (double)nf);
+        qsort(v, (size_t)nf, sizeof(double), cmp_double);
+        const double med = (nf % 2) ? v[(nf - 1) / 2] : (v[nf / 2 - 1] + v[nf / 2]) * 0.5;
+        for (int64_t k = 0; k < n; ++k) {
+            if ((filt ? filt[k] : 0) != f) continue;
+            u[k] = (sd == 0.0) ? 0.0 : (m[k] - med) / sd;
+        }
+    }
+    free(v);
+    return GCE_ORACLE_OK;
+}
 
 /* ---------------------------------------------------------------------------------------
  * S1  preprocess one light curve (north_star (2)): t0 = min t, dt = t - t0,

@@ -464,3 +464,78 @@ def test_overlap_special_cases_and_bounds(oracle):
     # enters two bins with weight 1/2: H(mixture) >= the weighted mean of the parts (concavity) and <= that mean + ln 2
     assert np.all(ov >= pl - 1e-12)
     assert np.all(ov <= pl + math.log(2) + 1e-12)
+
+
+# ------------------------------------------------------------------------------------------ N4: per-filter median / std
+def test_normalise_hand_examples(oracle):
+    """PAPER.md:96 (reading Q19): u = (m - median) / population std, per filter.  Closed forms by hand:
+    [1,2,3,4,10]: median 3, mean 4, var (9+4+1+0+36)/5 = 10;  [1,2,3,4]: median 2.5, var 1.25."""
+    u = oracle.normalise(np.array([1.0, 2.0, 3.0, 4.0, 10.0]))
+    np.testing.assert_allclose(u, (np.array([1.0, 2, 3, 4, 10]) - 3.0) / math.sqrt(10.0), rtol=1e-15)
+    u = oracle.normalise(np.array([4.0, 1.0, 3.0, 2.0]))
+    np.testing.assert_allclose(u, (np.array([4.0, 1, 3, 2]) - 2.5) / math.sqrt(1.25), rtol=1e-15)
+    # dyadic case, exact: symmetric +-2 -> median 0, std 2
+    assert np.array_equal(oracle.normalise(np.array([-2.0, 2.0, 2.0, -2.0])), np.array([-1.0, 1.0, 1.0, -1.0]))
+    # degenerate filters: one point, all equal -> 0 (no NaN)
+    assert np.array_equal(oracle.normalise(np.array([5.0])), np.zeros(1))
+    assert np.array_equal(oracle.normalise(np.array([7.0, 7.0, 7.0])), np.zeros(3))
+    assert oracle.normalise(np.zeros(0)).shape == (0,)
+
+
+def test_normalise_matches_numpy_per_filter(oracle):
+    """Library special case: numpy.median / numpy.std (ddof 0) on each filter's points; interleaved filters."""
+    rng = np.random.default_rng(11)
+    m = rng.normal(18.0, 0.4, 500)
+    f = rng.integers(0, 3, 500).astype(np.int32)
+    m[f == 1] += 1.3
+    m[f == 2] *= 0.5
+    u = oracle.normalise(m, f)
+    for k in range(3):
+        sel = f == k
+        np.testing.assert_allclose(u[sel], (m[sel] - np.median(m[sel])) / np.std(m[sel]), rtol=1e-12, atol=1e-13)
+        assert abs(np.median(u[sel])) < 1e-13 and abs(np.std(u[sel]) - 1.0) < 1e-12
+    # filter ids outside 0..7 are refused
+    with pytest.raises(Exception):
+        oracle.normalise(m, np.full(500, 8, dtype=np.int32))
+
+
+def test_single_filter_normalisation_does_not_change_the_bins(oracle):
+    """Reading Q2: equal-width bins over the data range are invariant under positive affine maps, so with ONE filter the
+    paper's median / std step leaves every magnitude bin where min/max normalisation puts it -- exactly on dyadic data,
+    and on random data except for points within rounding of a bin edge."""
+    m = np.array([-2.0, 2.0, 2.0, -2.0, -2.0, 2.0, 2.0, -2.0])   # median 0, std 2: u = m / 2 exactly
+    t = np.arange(m.size, dtype=np.float64)
+    raw = oracle.preprocess(t, m, 8)[2]
+    norm = oracle.preprocess(t, oracle.normalise(m), 8)[2]
+    assert np.array_equal(raw, norm) and set(raw) == {0, 7}
+    rng = np.random.default_rng(3)
+    mr = rng.normal(17.0, 0.3, 4000)
+    tr = np.arange(4000.0)
+    raw_r = oracle.preprocess(tr, mr, 10)[2]
+    norm_r = oracle.preprocess(tr, oracle.normalise(mr), 10)[2]
+    u = (mr - mr.min()) / (mr.max() - mr.min()) * 10
+    near_edge = np.abs(u - np.round(u)) < 1e-9
+    assert np.array_equal(raw_r[~near_edge], norm_r[~near_edge])
+    assert np.mean(raw_r == norm_r) > 0.999
+
+
+def test_two_filters_merged_into_one_light_curve(oracle):
+    """What the option is for: two filters offset by 0.9 mag merged into one light curve.  After the
+    per-filter median / std step both filters share one scale (median 0, std 1 each), the magnitude bins differ from the
+    min/max bins of the raw merged magnitudes, and the CE minimum on a dense local grid sits at the injected period."""
+    import gce_workloads as W
+    w, filt = W.two_filter_batch(5, n_lc=3, n_obs=400, n_p=500, n_pdot=1)
+    u = oracle.normalise_batch(w.mags, w.lc_offsets, filt)
+    for lc in range(3):
+        a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
+        for k in (0, 1):
+            sel = filt[a:b] == k
+            assert abs(np.median(u[a:b][sel])) < 1e-13 and abs(np.std(u[a:b][sel]) - 1.0) < 1e-12
+        raw_bins = oracle.preprocess(w.times[a:b], w.mags[a:b], 10)[2]
+        norm_bins = oracle.preprocess(w.times[a:b], u[a:b], 10)[2]
+        assert np.mean(raw_bins != norm_bins) > 0.3
+        P = w.truth["P"][lc]
+        periods = 1.0 / (1.0 / P + np.arange(-150, 151) / (3.0 * w.times[b - 1]))   # dense local grid around the truth
+        offs = np.array([0, b - a], dtype=np.int64)
+        ce_norm = oracle.ce_search(w.times[a:b], u[a:b], offs, periods, np.zeros(1), 20, 10)[0].ravel()
+        assert abs(int(np.argmin(ce_norm)) - 150) <= 1
