@@ -175,7 +175,8 @@ int gce_ce_debug_histogram(const double *times, const double *mags, const int64_
  * functions, called with the thread context the search builds for trial q (its R - 1 slot neighbours, slots sorted by
  * c where floors can be shared).  fold_mode selects which of the kernel's fold variants runs: GCE_CE_FOLD_AUTO = the one
  * the owning thread qualifies for, or one of them forced; out_fold_mode (device int32[1], may be NULL) receives the
- * variant used, or -1 -- and every bin is -1 -- when the forced variant's precondition does not hold for this trial. */
+ * variant used, or -1 -- and every bin is -1 -- when the forced variant's precondition does not hold for this trial.
+ * prm->normalise is ignored (the magnitude bins are those of min/max scaling of `mags` as given). */
 #define GCE_CE_FOLD_AUTO 0
 #define GCE_CE_FOLD_PLAIN 1     /* j = floor(y) - n_phi floor(x), one floor(x) per trial; needs |y| < 2^51        */
 #define GCE_CE_FOLD_PAIR 2      /* the two trials of a counter word share floor(x); needs them within one cycle  */

@@ -129,7 +129,7 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
 }
 
 struct Layout {
-    size_t pts, seg, info, ltab, part_S, part_q, part_stats, total;
+    size_t pts, seg, info, ltab, part_S, part_q, part_stats, mnorm, total;
     int ltab_n;
 };
 
@@ -151,6 +151,8 @@ Layout make_layout(int64_t total_points, int32_t n_lc, int64_t n_trials, int64_t
     L.part_q = o; o = align_up(o + sizeof(int64_t) * parts, 256);
     L.part_stats = o;
     if (prm->want_stats) o = align_up(o + sizeof(uint64_t) * kStatWords * (size_t)(n_lc > 0 ? n_lc : 1) * (size_t)p.jobs_per_lc, 256);
+    L.mnorm = o;
+    if (prm->normalise) o = align_up(o + sizeof(double) * (size_t)(total_points > 0 ? total_points : 1), 256);
     L.total = o;
     return L;
 }
@@ -237,8 +239,8 @@ int gce_ce_last_cuda_error(void) { return g_last_cuda_error; }
 
 int gce_ce_launch_count(int32_t n_lc, int64_t n_p, const gce_ce_params *prm, int partial) {
     if (!prm || n_lc <= 0) return 0;
-    // preprocess (+ table), search (when the grid is not empty), [merge_topk], [merge_stats: Eq. 5 and every partial blob]
-    return 1 + (n_p > 0 ? 1 : 0) + (prm->top_k > 0 ? 1 : 0) + ((prm->want_stats || partial) ? 1 : 0);
+    // [normalise], preprocess (+ table), search (when the grid is not empty), [merge_topk], [merge_stats: Eq. 5 and every partial blob]
+    return (prm->normalise ? 1 : 0) + 1 + (n_p > 0 ? 1 : 0) + (prm->top_k > 0 ? 1 : 0) + ((prm->want_stats || partial) ? 1 : 0);
 }
 
 int gce_ce_workspace_bytes(int64_t total_points, int32_t n_lc, int64_t n_p, int64_t n_pdot, const gce_ce_params *prm,
@@ -319,7 +321,15 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     sp.part_stats = (!dump && prm->want_stats) ? reinterpret_cast<uint64_t *>(ws + L.part_stats) : nullptr;
     sp.out_counts = out_counts; sp.out_ce_at = out_ce_at;
 
-    k_preprocess<<<n_lc + (L.ltab_n + 255) / 256, 256, 0, st>>>(times, mags, lc_offsets, n_lc, prm->n_mag_bins, pts, seg, info,
+    const double *mags_used = mags;
+    if (prm->normalise && total_points > 0) {  // S0 (N4): per-filter median / std into the workspace
+        double *mnorm = reinterpret_cast<double *>(ws + L.mnorm);
+        k_normalise<<<n_lc, 256, 0, st>>>(mags, prm->filter_ids, lc_offsets, mnorm);
+        cudaError_t en = cudaGetLastError();
+        if (en != cudaSuccess) return cuda_fail(en);
+        mags_used = mnorm;
+    }
+    k_preprocess<<<n_lc + (L.ltab_n + 255) / 256, 256, 0, st>>>(times, mags_used, lc_offsets, n_lc, prm->n_mag_bins, pts, seg, info,
                                                               ltab, L.ltab_n, table_shift(L.ltab_n), mult, (int)max_points);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
@@ -488,6 +498,9 @@ int gce_ce_validate_host(const double *times, const double *mags, const int64_t 
     if (total > 0 && (!times || !mags)) return GCE_CE_ERR_POINTER;
     for (int64_t k = 0; k < total; ++k)
         if (!(times[k] - times[k] == 0.0) || !(mags[k] - mags[k] == 0.0)) return GCE_CE_ERR_RANGE;  // NaN / inf
+    if (prm->normalise && prm->filter_ids)  // a HOST pointer here
+        for (int64_t k = 0; k < total; ++k)
+            if (prm->filter_ids[k] < 0 || prm->filter_ids[k] >= GCE_CE_MAX_FILTERS) return GCE_CE_ERR_RANGE;
     if (n_p > 0 && !periods) return GCE_CE_ERR_POINTER;
     if (!pdots) return GCE_CE_ERR_POINTER;
     for (int64_t i = 0; i < n_p; ++i)
@@ -576,8 +589,11 @@ struct HostCall {
 // cube slice to the caller's buffer, so the device-to-host transfer of the cube overlaps the search of the next chunk.
 static int search_host_pipelined(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
                                  int64_t total, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
-                                 const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                                 const gce_ce_params *prm_in, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
                                  double *out_stats, int n_chunks) {
+    gce_ce_params prm_dev = *prm_in;  // filter_ids: the caller's HOST pointer is replaced by a device copy below
+    const gce_ce_params *prm = &prm_dev;
+    const int32_t *filt_host = prm_in->normalise ? prm_in->filter_ids : nullptr;
     const size_t esz = prm->ce_fp64 ? 8 : 4;
     const int64_t chunk = (n_p + n_chunks - 1) / n_chunks;
     const size_t k = (size_t)prm->top_k, W = gce_ce_partial_words(prm->top_k);
@@ -606,6 +622,12 @@ static int search_host_pipelined(const double *times, const double *mags, const 
         CU(hc.alloc(&d_sl[0], slice_bytes)); CU(hc.alloc(&d_sl[1], slice_bytes));
         CU(hc.alloc(&d_part, 8 * W * (size_t)n_lc * (size_t)n_chunks)); CU(hc.alloc(&d_idx, 8 * (size_t)n_lc * k));
         CU(hc.alloc(&d_bce, 4 * (size_t)n_lc * k)); CU(hc.alloc(&d_st, 32 * (size_t)n_lc));
+        if (filt_host) {
+            void *d_filt = nullptr;
+            CU(hc.alloc(&d_filt, 4 * (size_t)total));
+            CU(cudaMemcpyAsync(d_filt, filt_host, 4 * (size_t)total, cudaMemcpyHostToDevice, st));
+            prm_dev.filter_ids = static_cast<const int32_t *>(d_filt);
+        }
         CU(cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
         CU(cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
         CU(cudaMemcpyAsync(d_off, lc_offsets, 8 * (size_t)(n_lc + 1), cudaMemcpyHostToDevice, st));
@@ -691,6 +713,12 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
         CU(hc.alloc(&d_pd, 8 * (size_t)n_pdot)); CU(hc.alloc(&d_ws, ws_bytes));
         CU(hc.alloc(&d_ce, ce_bytes)); CU(hc.alloc(&d_idx, 8 * (size_t)n_lc * k));
         CU(hc.alloc(&d_bce, 4 * (size_t)n_lc * k)); CU(hc.alloc(&d_st, 32 * (size_t)n_lc));
+        if (prm_in->normalise && prm_in->filter_ids && total) {  // the caller's HOST filter ids -> device copy
+            void *d_filt = nullptr;
+            CU(hc.alloc(&d_filt, 4 * (size_t)total));
+            CU(cudaMemcpyAsync(d_filt, prm_in->filter_ids, 4 * (size_t)total, cudaMemcpyHostToDevice, st));
+            prm_local.filter_ids = static_cast<const int32_t *>(d_filt);
+        }
         if (total) {
             CU(cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, st));
             CU(cudaMemcpyAsync(d_m, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, st));

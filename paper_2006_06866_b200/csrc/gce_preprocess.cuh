@@ -11,6 +11,95 @@ __device__ __forceinline__ int64_t ltab_entry(int k, int shift) {
     return k < 2 ? 0 : __double2ll_rn(ldexp((double)k * log((double)k), shift));
 }
 
+// ------------------------------------------------------------------------------------------------ S0 (optional, N4)
+// The paper's normalisation (reading Q19): per light curve and per filter, u = (m - median) / sd
+// with sd the population standard deviation, so that filters can be merged into one light curve; S1 then bins the
+// merged u over its range.  Frozen arithmetic: the median is an order statistic (the mean of the two middle values,
+// (a + b) * 0.5, when the count is even); mean and sum of squares are SEQUENTIAL sums over the filter's points in
+// light-curve order, one rounding per operation (a thread per filter walks the light curve); sd == 0 -> u = 0.
+// One CTA per light curve.  Order statistics by an 8-pass radix select over the order-preserving 64-bit keys.
+__device__ __forceinline__ unsigned long long order_key(double v) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double key_value(unsigned long long k) {
+    const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)b);
+}
+
+__global__ void __launch_bounds__(256) k_normalise(const double *__restrict__ mags, const int32_t *__restrict__ filt,
+                                                   const int64_t *__restrict__ lc_offsets, double *__restrict__ out) {
+    __shared__ unsigned int hist[256];
+    __shared__ unsigned long long sh_prefix;
+    __shared__ long long sh_rank;
+    __shared__ int sh_cnt[GCE_CE_MAX_FILTERS];
+    __shared__ double sh_med[GCE_CE_MAX_FILTERS], sh_sd[GCE_CE_MAX_FILTERS];
+    const int lc = blockIdx.x, tid = threadIdx.x;
+    const int64_t off = lc_offsets[lc];
+    const int64_t n = lc_offsets[lc + 1] - off;
+    if (n <= 0) return;
+    const double *m = mags + off;
+    const int32_t *f = filt ? filt + off : nullptr;
+    if (tid < GCE_CE_MAX_FILTERS) sh_cnt[tid] = 0;
+    __syncthreads();
+    for (int64_t k = tid; k < n; k += blockDim.x) atomicAdd(&sh_cnt[(f ? f[k] : 0) & (GCE_CE_MAX_FILTERS - 1)], 1);
+    __syncthreads();
+    // sequential mean and standard deviation: thread g walks the light curve for filter g
+    if (tid < GCE_CE_MAX_FILTERS && sh_cnt[tid] > 0) {
+        const double nf = (double)sh_cnt[tid];
+        double sum = 0.0;
+        for (int64_t k = 0; k < n; ++k)
+            if (((f ? f[k] : 0) & (GCE_CE_MAX_FILTERS - 1)) == tid) sum = __dadd_rn(sum, m[k]);
+        const double mean = __ddiv_rn(sum, nf);
+        double ss = 0.0;
+        for (int64_t k = 0; k < n; ++k)
+            if (((f ? f[k] : 0) & (GCE_CE_MAX_FILTERS - 1)) == tid) {
+                const double d = __dsub_rn(m[k], mean);
+                ss = __dadd_rn(ss, __dmul_rn(d, d));
+            }
+        sh_sd[tid] = __dsqrt_rn(__ddiv_rn(ss, nf));
+    }
+    // medians: radix select of the two middle order statistics, filter by filter (block-wide)
+    for (int g = 0; g < GCE_CE_MAX_FILTERS; ++g) {
+        const int nf = sh_cnt[g];
+        if (nf == 0) continue;  // uniform
+        double mid[2];
+        for (int h = 0; h < 2; ++h) {
+            const long long want = h == 0 ? (nf - 1) / 2 : nf / 2;
+            if (h == 1 && want == (nf - 1) / 2) { mid[1] = mid[0]; break; }
+            if (tid == 0) { sh_prefix = 0ull; sh_rank = want; }
+            for (int pass = 7; pass >= 0; --pass) {
+                hist[tid] = 0u;  // 256 threads
+                __syncthreads();
+                const unsigned long long prefix = sh_prefix;
+                for (int64_t k = tid; k < n; k += blockDim.x) {
+                    if (((f ? f[k] : 0) & (GCE_CE_MAX_FILTERS - 1)) != g) continue;
+                    const unsigned long long key = order_key(m[k]);
+                    if (pass == 7 || (key >> (8 * (pass + 1))) == prefix) atomicAdd(&hist[(key >> (8 * pass)) & 0xffu], 1u);
+                }
+                __syncthreads();
+                if (tid == 0) {
+                    long long r = sh_rank;
+                    int b = 0;
+                    while (r >= (long long)hist[b]) { r -= hist[b]; ++b; }
+                    sh_rank = r;
+                    sh_prefix = (prefix << 8) | (unsigned long long)b;
+                }
+                __syncthreads();
+            }
+            mid[h] = key_value(sh_prefix);
+            __syncthreads();
+        }
+        if (tid == 0) sh_med[g] = (nf & 1) ? mid[0] : __dmul_rn(__dadd_rn(mid[0], mid[1]), 0.5);
+    }
+    __syncthreads();
+    for (int64_t k = tid; k < n; k += blockDim.x) {
+        const int g = (f ? f[k] : 0) & (GCE_CE_MAX_FILTERS - 1);
+        const double sd = sh_sd[g];
+        out[off + k] = sd == 0.0 ? 0.0 : __ddiv_rn(__dsub_rn(m[k], sh_med[g]), sd);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ S1
 // CTAs 0 .. n_lc-1: one per light curve.  Output points are permuted so equal magnitude bins are contiguous (counts do
 // not depend on point order); seg[lc][i] is the first point of magnitude bin i, seg[lc][n_m] = N.

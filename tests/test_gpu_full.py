@@ -570,3 +570,77 @@ def test_pdot_zero_grids_fine_and_coarse(gce, oracle, n_phi, overlap, step):
                        want_cube=True, ce_fp64=True, overlap=overlap)
     torch.cuda.synchronize()
     assert torch.equal(res_r.ce.flip(1), res.ce)
+
+
+# ------------------------------------------------------------------------------------------ N4: per-filter median / std
+def test_two_filter_normalisation_matches_the_oracle(gce, oracle):
+    """NEXT item N4: normalise = 1 with per-point filter ids.  The GPU's S0 follows the same frozen
+    arithmetic as oracle.normalise (order-statistic median, sequential sums), so magnitude bins and counts are bit-exact
+    and the cube agrees at the fp64 tolerance; selection and Eq. 5 follow."""
+    w, filt = W.two_filter_batch(21, n_lc=5, n_obs=401, n_p=500, n_pdot=4)
+    u = oracle.normalise_batch(w.mags, w.lc_offsets, filt)
+    ref = oracle.ce_search(w.times, u, w.lc_offsets, w.periods, w.pdots, 20, 10)
+    raw = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 10)
+    assert np.max(np.abs(ref - raw)) > 1e-2          # the option changes the result on a two-filter light curve
+    args = (dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots), 20, 10)
+    res = gce.search(*args, top_k=3, want_cube=True, ce_fp64=True, want_stats=True, normalise=True, filter_ids=dev(filt))
+    torch.cuda.synchronize()
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    for lc in range(w.n_lc):
+        assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), 3, RTOL64, oracle)
+    # bit-exact counts through the normalised magnitudes
+    q = torch.tensor([0, 17, 500 * 4 - 1], dtype=torch.int64, device="cuda")
+    fdev = dev(filt)   # the params hold a raw pointer: keep the tensor alive
+    prm = gce.make_params(20, 10, normalise=True, filter_ids=fdev)
+    counts = torch.empty((w.n_lc, 3, 20, 10), dtype=torch.int32, device="cuda")
+    ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, 500, 4, prm), dtype=torch.uint8, device="cuda")
+    gce.gce_ce_debug_histogram(dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots), prm, q, counts, None, ws)
+    torch.cuda.synchronize()
+    for lc in range(w.n_lc):
+        a, b = int(w.lc_offsets[lc]), int(w.lc_offsets[lc + 1])
+        refc = oracle.histogram(w.times[a:b], u[a:b], w.periods, w.pdots, 20, 10, q.cpu().numpy())
+        assert np.array_equal(counts[lc].cpu().numpy().astype(np.int64), refc)
+    # host entry: filter ids as a host array
+    ce_h = np.empty((w.n_lc, 500, 4), dtype=np.float64)
+    idx_h = np.empty((w.n_lc, 3), dtype=np.int64)
+    gce.gce_ce_search_host(w.times, w.mags, w.lc_offsets, w.periods, w.pdots,
+                           gce.make_params(20, 10, top_k=3, ce_fp64=True, normalise=True, filter_ids=torch.from_numpy(filt)),
+                           ce_h, idx_h, None)
+    assert np.array_equal(ce_h, res.ce.cpu().numpy()) and np.array_equal(idx_h, res.best_idx.cpu().numpy())
+
+
+@pytest.mark.parametrize("n_obs,n_filters", [(1, 1), (2, 1), (777, 1), (5000, 3), (20001, 8)])
+def test_normalised_magnitude_bins_are_bit_exact(gce, oracle, n_obs, n_filters):
+    """S0 + S1 alone: with n_phase_bins = 1 every count table is the magnitude histogram of the normalised light curve
+    (independent of the trial), compared bit for bit with the oracle's bins; even / odd filter sizes, a filter with one
+    point, ties, light curves longer than one radix-select pass's worth of threads."""
+    rng = np.random.default_rng(n_obs * 10 + n_filters)
+    m = np.round(rng.normal(17.0, 0.5, n_obs), 2)               # rounded: many exact ties around the median
+    f = rng.integers(0, n_filters, n_obs).astype(np.int32)
+    if n_obs > 10:
+        f[0] = n_filters - 1
+        m[f == 0] += 2.5
+    t = np.sort(rng.uniform(0, 1e7, n_obs))
+    offs = np.array([0, n_obs], dtype=np.int64)
+    u = oracle.normalise(m, f)
+    mb = oracle.preprocess(t, u, 13)[2]
+    fdev = dev(f)
+    prm = gce.make_params(1, 13, normalise=True, filter_ids=fdev)
+    counts = torch.empty((1, 1, 1, 13), dtype=torch.int32, device="cuda")
+    ws = torch.empty(gce.gce_ce_workspace_bytes(n_obs, 1, 1, 1, prm), dtype=torch.uint8, device="cuda")
+    gce.gce_ce_debug_histogram(dev(t), dev(m), dev(offs), dev(np.array([500.0])), dev(np.zeros(1)), prm,
+                               torch.zeros(1, dtype=torch.int64, device="cuda"), counts, None, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(counts.cpu().numpy().ravel(), np.bincount(mb, minlength=13))
+
+
+def test_one_filter_normalisation_equals_min_max(gce):
+    """Reading Q2 on the GPU: with one filter the paper's normalisation leaves the search result unchanged up to points
+    within rounding of a magnitude-bin edge -- here: the same best trials on C2-like light curves."""
+    w = W.make("C2", n_lc=6, n_p=1500)
+    args = (dev(w.times), dev(w.mags), dev(w.lc_offsets), dev(w.periods), dev(w.pdots), 20, 10)
+    a = gce.search(*args, top_k=1, want_cube=True, ce_fp64=True)
+    b = gce.search(*args, top_k=1, want_cube=True, ce_fp64=True, normalise=True)
+    torch.cuda.synchronize()
+    assert torch.equal(a.best_idx, b.best_idx)
+    assert float((a.ce - b.ce).abs().max()) < 0.02   # a handful of edge points may move by one bin
