@@ -48,6 +48,7 @@ UNIT = "point-folds/s"
 FP64_LANES_PER_SM_CLK = 64       # B200 FP64 pipe: 64 lane-ops / SM / clk (probe-measured)
 N_SM = 148
 OVERLAP = [False]   # set from --overlap; the oracle legs time the same binning
+PROBED = {}         # gce_ce_probe_rate results of this run (rank 0)
 SHARED_WAVEFRONTS_PER_SM_CLK = 1   # shared-memory data pipe: 1 wavefront / SM / clk (ncu's own denominator)
 DEFAULT_CONFIG = "C5"              # BASELINE.json:configs[4]: the largest single-GPU configuration
 SECONDARY_CONFIG = "C3"            # configs[2]: the other P-Pdot grid of the north_star's roofline target
@@ -118,12 +119,14 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def make_workload(name, rank, shrink):
+def make_workload(name, rank, shrink, n_pdot=0):
     kw = {}
     if shrink:  # --quick: same ranges, smaller grid (for smoke-testing the bench itself; never a reported number)
         kw = {"C1": {}, "C2": dict(n_lc=8, n_p=2000), "C3": dict(n_lc=4, n_p=2000, n_pdot=64),
               "C4": dict(n_lc=16, n_p=4000), "C5": dict(n_lc=2, n_p=512, n_pdot=32),
               "P1": dict(n_lc=4, n_p=20000, n_pdot=32)}[name]
+    if name == "P1" and n_pdot:
+        kw = dict(kw, n_pdot=n_pdot)
     if rank > 0:
         # weak scaling: every rank owns a batch of the same shape; rank r re-draws it from seed + 1000 r
         kw = dict(kw, seed={"C1": 0, "C2": 1, "C3": 2, "C4": 3, "C5": 4, "P1": 9}[name] + 1000 * rank)
@@ -183,7 +186,7 @@ def run_reference(args):
     if name == "P1":
         args.overlap = True
         OVERLAP[0] = True
-    w = apply_binning(make_workload(name, 0, args.quick), args)
+    w = apply_binning(make_workload(name, 0, args.quick, args.n_pdot), args)
     per_step = max(1.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
     sample, desc = oracle_sample(w, per_step)
     for _ in range(args.warmup):
@@ -336,14 +339,20 @@ def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline)
             "peak": FP64_LANES_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9, "unit": "G FP64 lane-ops/s",
             "algorithmic_per_point_fold": fp64_ops,
             "peak_source": f"nominal 64 FP64 lanes/SM/clk x 148 SMs x {sm_max:.0f} MHz (max SM clock, {peaks_src} MEASURED_PEAKS.json, "
-                           "which has no FP64 entry; a probe of independent DMUL/DADD chains reached 62.0-62.6 lanes/SM/clk, "
-                           "profiles/r2_peaks.md, so the nominal figure is the stricter denominator)"}
+                           "which has no FP64 entry); the library's probe of independent DMUL/DADD chains (gce_ce_probe_rate, "
+                           "probe_measured_per_sm_clk) stays just below it, so the nominal figure is the stricter denominator"}
     wf = algorithmic_shared_wavefronts_per_pointfold(w)
     shm = {"bound": "alu", "pipe": "shared-memory wavefronts", "achieved": wf * pf_s / 1e9,
            "peak": SHARED_WAVEFRONTS_PER_SM_CLK * N_SM * sm_max * 1e6 / 1e9, "unit": "G wavefronts/s",
            "algorithmic_per_point_fold": wf,
            "peak_source": f"1 shared-memory wavefront/SM/clk x 148 SMs x {sm_max:.0f} MHz (the denominator of ncu's "
-                          "l1tex__data_pipe_lsu_wavefronts_mem_shared pct_of_peak; DESIGN.md section 7)"}
+                          "l1tex__data_pipe_lsu_wavefronts_mem_shared pct_of_peak; DESIGN.md section 7); probe_measured_per_sm_clk is "
+                          "the library's conflict-free RED.shared probe"}
+    if not PROBED:   # once per run: the per-SM rates behind the two denominators, measured on this GPU by the library's probe
+        PROBED["fp64"] = gce.gce_ce_probe_rate(gce.binding.PROBE_FP64)
+        PROBED["shared"] = gce.gce_ce_probe_rate(gce.binding.PROBE_SHARED)
+    fp64["probe_measured_per_sm_clk"], fp64["nominal_per_sm_clk"] = PROBED["fp64"], FP64_LANES_PER_SM_CLK
+    shm["probe_measured_per_sm_clk"], shm["nominal_per_sm_clk"] = PROBED["shared"], SHARED_WAVEFRONTS_PER_SM_CLK
     for r in (fp64, shm):
         r["frac"] = r["achieved"] / r["peak"]
         r["ceiling_point_folds_per_s"] = r["peak"] * 1e9 / r["algorithmic_per_point_fold"]
@@ -399,7 +408,7 @@ def run_ours(args):
     if name == "P1":
         args.overlap = True   # the paper's production binning
         OVERLAP[0] = True
-    w = apply_binning(make_workload(name, rank, args.quick), args)
+    w = apply_binning(make_workload(name, rank, args.quick, args.n_pdot), args)
     line = measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline=not args.no_cpu_baseline)
     if args.config is None:
         # the other P-Pdot grid the north_star's roofline target is stated on, same K / W, its own record
@@ -476,6 +485,7 @@ def main():
     ap.add_argument("--n-phase-bins", type=int, default=0, help="override the config's phase bin count (named in config)")
     ap.add_argument("--n-mag-bins", type=int, default=0, help="override the config's magnitude bin count")
     ap.add_argument("--overlap", action="store_true", help="50 %% overlapping phase bins (N2, PAPER.md:106)")
+    ap.add_argument("--n-pdot", type=int, default=0, help="P1 only: 32 / 128 / 512 log-spaced Pdot values (PAPER.md:170)")
     ap.add_argument("--sweep", action="store_true", help="the paper's Fig. 3 sweep instead of the benchmark line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)

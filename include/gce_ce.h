@@ -198,6 +198,14 @@ int gce_ce_validate_host(const double *times_host, const double *mags_host, cons
  * enqueues for these arguments (for launch accounting). */
 int gce_ce_launch_count(int32_t n_lc, int64_t n_p, const gce_ce_params *prm_host, int partial);
 
+/* Diagnostic, synchronous: measures on the current device the per-SM issue rate a roofline denominator assumes, with a
+ * probe kernel of 1024 threads per SM timed by the SM's own clock counter (so the figure is per clock, whatever the
+ * clock).  GCE_CE_PROBE_FP64: FP64 lane-operations per SM per clock from independent DADD / DMUL chains (nominal 64 on
+ * B200).  GCE_CE_PROBE_SHARED: shared-memory wavefronts per SM per clock from conflict-free RED.shared (nominal 1). */
+#define GCE_CE_PROBE_FP64 0
+#define GCE_CE_PROBE_SHARED 1
+int gce_ce_probe_rate(int32_t kind, double *rate_host);
+
 const char *gce_ce_strerror(int code);
 int gce_ce_last_cuda_error(void); /* cudaError_t of the most recent GCE_CE_ERR_CUDA on this thread */
 const char *gce_ce_version(void);

@@ -51,18 +51,20 @@ _lib.gce_ce_merge_partials_to_partial.argtypes = [_vp, _i32, _i32, C.POINTER(Par
 _lib.gce_ce_merge_partials_to_partial.restype = C.c_int
 _lib.gce_ce_validate_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params)]
 _lib.gce_ce_launch_count.argtypes = [_i32, _i64, C.POINTER(Params), C.c_int]
+_lib.gce_ce_probe_rate.argtypes = [_i32, C.POINTER(C.c_double)]
 _lib.gce_ce_strerror.argtypes = [C.c_int]
 _lib.gce_ce_strerror.restype = C.c_char_p
 _lib.gce_ce_version.restype = C.c_char_p
 for _f in ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
            "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_last_cuda_error",
-           "gce_ce_search_partial", "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release"):
+           "gce_ce_search_partial", "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release",
+           "gce_ce_probe_rate"):
     getattr(_lib, _f).restype = C.c_int
 
 EXPORTS = ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
            "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_strerror",
            "gce_ce_last_cuda_error", "gce_ce_version", "gce_ce_partial_words", "gce_ce_search_partial",
-           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release")
+           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release", "gce_ce_probe_rate")
 
 
 class GceError(RuntimeError):
@@ -162,6 +164,16 @@ def gce_ce_host_release() -> None:
     """Return the cached device memory of the host entry points to the driver."""
     _lib.gce_ce_host_release.restype = C.c_int
     _check(_lib.gce_ce_host_release())
+
+
+PROBE_FP64, PROBE_SHARED = 0, 1
+
+
+def gce_ce_probe_rate(kind) -> float:
+    """Measured per-SM issue rate on the current device: FP64 lane-ops / SM / clk or shared wavefronts / SM / clk."""
+    out = C.c_double(0.0)
+    _check(_lib.gce_ce_probe_rate(int(kind), C.byref(out)))
+    return float(out.value)
 
 
 def gce_ce_partial_words(top_k) -> int:

@@ -25,10 +25,13 @@
 //
 // This translation unit must be compiled with -fmad=false; the fold additionally uses explicit _rn/_rd
 // intrinsics, which are never contracted.
+#include <vector>
+
 #include "gce_common.cuh"
 #include "gce_preprocess.cuh"
 #include "gce_debug.cuh"
 #include "gce_select.cuh"
+#include "gce_probe.cuh"
 
 namespace {
 
@@ -479,6 +482,37 @@ int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return GCE_CE_OK;
+}
+
+int gce_ce_probe_rate(int32_t kind, double *rate_host) {
+    if (!rate_host) return GCE_CE_ERR_POINTER;
+    if (kind != GCE_CE_PROBE_FP64 && kind != GCE_CE_PROBE_SHARED) return GCE_CE_ERR_RANGE;
+    int dev = 0, n_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    void *sink = nullptr;
+    long long *out = nullptr;
+    int rc = GCE_CE_OK;
+    std::vector<long long> h((size_t)2 * n_sm);
+    do {
+        if ((e = cudaMalloc(&sink, (size_t)n_sm * 1024 * sizeof(double))) != cudaSuccess) { rc = cuda_fail(e); break; }
+        if ((e = cudaMalloc(&out, sizeof(long long) * 2 * (size_t)n_sm)) != cudaSuccess) { rc = cuda_fail(e); break; }
+        for (int pass = 0; pass < 2; ++pass) {  // the first pass warms up (clocks, instruction cache)
+            const int iters = pass == 0 ? 200 : 20000;
+            if (kind == GCE_CE_PROBE_FP64) k_probe_fp64<<<n_sm, 1024>>>(static_cast<double *>(sink), out, iters, 1.0000001);
+            else k_probe_shared<<<n_sm, 1024>>>(static_cast<unsigned *>(sink), out, iters);
+            if ((e = cudaGetLastError()) != cudaSuccess) break;
+        }
+        if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+        if ((e = cudaMemcpy(h.data(), out, sizeof(long long) * 2 * (size_t)n_sm, cudaMemcpyDeviceToHost)) != cudaSuccess) { rc = cuda_fail(e); break; }
+        double sum = 0.0;
+        for (int i = 0; i < n_sm; ++i) sum += (double)h[2 * i] / (double)(h[2 * i + 1] > 0 ? h[2 * i + 1] : 1);
+        *rate_host = sum / n_sm;  // mean over the SMs of operations per clock of that SM
+    } while (0);
+    if (sink) cudaFree(sink);
+    if (out) cudaFree(out);
+    return rc;
 }
 
 int gce_ce_validate_host(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
