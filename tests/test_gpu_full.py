@@ -405,6 +405,14 @@ def test_fused_significance_degenerate_and_split_invariance(gce, oracle):
                       want_cube=False, want_stats=True)
     torch.cuda.synchronize()
     assert np.array_equal(res2.stats.cpu().numpy()[0], st[2])
+    # a one-trial grid on a long light curve: N * CE * 2^42 needs more than 53 bits, mean and min must still be the same
+    # number and rho NaN (not +-inf from two differently rounded conversions)
+    t5 = np.sort(rng.uniform(0, 1e7, 5000)); m5 = rng.normal(size=5000)
+    res3 = gce.search(d(t5), d(m5), d(np.array([0, 5000])), d(np.array([733.0])), d(np.zeros(1)), 20, 10, top_k=1,
+                      want_cube=True, ce_fp64=True, want_stats=True)
+    torch.cuda.synchronize()
+    s3 = res3.stats.cpu().numpy()[0]
+    assert s3[0] == s3[2] == float(res3.ce.ravel()[0]) > 1.0 and s3[1] == 0.0 and np.isnan(s3[3])
 
 
 def test_c4_full_stats_sampled_light_curves(gce, oracle):
