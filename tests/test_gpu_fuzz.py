@@ -1,6 +1,7 @@
 """Seeded differential test of the CUDA path against the oracle over random shapes: bin counts 1..64, 1..9 Pdot values of
 either sign, ragged batches incl. empty and very short light curves, plain / overlapping bins, fp32 / fp64 cubes, top-k
-0..32, Eq. 5 on and off.  Every kernel variant (R = 2 / 4, shared or distinct periods, compile-time and generic n_phi,
+0..32, Eq. 5 on and off, the 32-bit counter kernels (forced through max_lc_points), the per-filter median / std
+normalisation with 1..8 filters.  Every kernel variant (R = 2 / 4, shared or distinct periods, compile-time and generic n_phi,
 register and shared-memory marginals, shared floors) is reached by some case."""
 import numpy as np
 import pytest
@@ -44,22 +45,40 @@ def _case(seed):
         pdots = np.sort(pdots)
     overlap = bool(rng.random() < 0.35)
     top_k = int(rng.choice([0, 1, 3, 5, 32]))
+    fp64, stats = bool(rng.random() < 0.6), bool(rng.random() < 0.5)
+    # drawn last so that the earlier cases keep their shapes: 32-bit counters although no light curve is long (the
+    # announced bound just has to exceed the 16-bit range), and the paper's normalisation with per-point filter ids
+    wide = bool(rng.random() < 0.25)
+    filt = None
+    if rng.random() < 0.3:
+        filt = rng.integers(0, int(rng.integers(1, 9)), size=times.size).astype(np.int32)
     return dict(times=times, mags=mags, offs=offs, periods=periods, pdots=np.ascontiguousarray(pdots), n_phi=n_phi, n_m=n_m,
-                overlap=overlap, top_k=top_k, fp64=bool(rng.random() < 0.6), stats=bool(rng.random() < 0.5))
+                overlap=overlap, top_k=top_k, fp64=fp64, stats=stats, wide=wide, filt=filt)
 
 
 @pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("GCE_FUZZ_N", "48"))))
 def test_random_shapes_match_oracle(gce, oracle, seed):
     c = _case(seed)
-    ref = oracle.ce_search(c["times"], c["mags"], c["offs"], c["periods"], c["pdots"], c["n_phi"], c["n_m"],
+    mags_ref = c["mags"] if c["filt"] is None else oracle.normalise_batch(c["mags"], c["offs"], c["filt"])
+    ref = oracle.ce_search(c["times"], mags_ref, c["offs"], c["periods"], c["pdots"], c["n_phi"], c["n_m"],
                            overlap=c["overlap"])
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    res = gce.search(d(c["times"]), d(c["mags"]), d(c["offs"]), d(c["periods"]), d(c["pdots"]), c["n_phi"], c["n_m"],
-                     top_k=c["top_k"], want_cube=True, ce_fp64=c["fp64"], want_stats=c["stats"], overlap=c["overlap"])
+    n_lc = c["offs"].size - 1
+    n_p, n_pdot, k = c["periods"].size, c["pdots"].size, c["top_k"]
+    fdev = None if c["filt"] is None else d(c["filt"])
+    prm = gce.make_params(c["n_phi"], c["n_m"], top_k=k, ce_fp64=c["fp64"], want_stats=c["stats"], overlap=c["overlap"],
+                          max_lc_points=70000 if c["wide"] else 0, normalise=fdev is not None, filter_ids=fdev)
+    res = gce.SearchResult(
+        torch.empty((n_lc, n_p, n_pdot), dtype=torch.float64 if c["fp64"] else torch.float32, device="cuda"),
+        torch.empty((n_lc, k), dtype=torch.int64, device="cuda") if k else None,
+        torch.empty((n_lc, k), dtype=torch.float32, device="cuda") if k else None,
+        torch.empty((n_lc, 4), dtype=torch.float64, device="cuda") if c["stats"] else None)
+    ws = torch.empty(gce.gce_ce_workspace_bytes(c["times"].size, n_lc, n_p, n_pdot, prm), dtype=torch.uint8, device="cuda")
+    gce.gce_ce_search(d(c["times"]), d(c["mags"]), d(c["offs"]), d(c["periods"]), d(c["pdots"]), prm, res.ce, res.best_idx,
+                      res.best_ce, res.stats, ws)
     torch.cuda.synchronize()
     rtol = RTOL64 if c["fp64"] else RTOL32
     assert_ce_close(res.ce.cpu().numpy(), ref, rtol)
-    n_lc = c["offs"].size - 1
     if c["top_k"]:
         for lc in range(n_lc):
             assert_topk_matches(ref[lc], res.best_idx[lc].cpu().numpy(), res.best_ce[lc].cpu().numpy(), c["top_k"], rtol,
