@@ -68,7 +68,7 @@ typedef struct gce_ce_params {
     int32_t want_stats;   /* 1: out_stats receives the Eq. 5 statistics (requires out_stats)      */
     int32_t overlap;      /* 0: plain bins (hot path).  1: 50 % overlapping phase bins (:106, :162):
                            * n_phase_bins bins of width 2/n_phase_bins, bin k = plain cells k-1 and k (cyclic),
-                           * every point counted twice, p = c / 2N.  The debug calls ignore it.            */
+                           * every point counted twice, p = c / 2N.  gce_ce_debug_bins ignores it.          */
     int32_t max_lc_points; /* 0: every light curve has at most GCE_CE_MAX_POINTS (_OVERLAP) points.  Larger (up to
                            * GCE_CE_MAX_POINTS_WIDE): an upper bound on the longest light curve of this call -- the
                            * search then runs with 32-bit counters and a k ln k table of that length (the paper's

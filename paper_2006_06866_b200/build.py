@@ -45,12 +45,24 @@ def _deps():
     return [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh"))] + [HDR, os.path.abspath(__file__)]
 
 
+def _code_only(text: str) -> str:
+    """C / C++ source with comments and blank space removed, so that editing documentation does not change the hash."""
+    import re
+    text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+    text = re.sub(r"//[^\n]*", " ", text)
+    return " ".join(text.split())
+
+
 def source_hash() -> str:
-    """SHA-256 over the sources the library is built from (bench.py ties ncu-derived numbers to it)."""
+    """SHA-256 over what the library's code is built from -- the csrc files and the header without their comments, the
+    compiler flags and the family list (bench.py ties ncu-derived numbers to it)."""
     h = hashlib.sha256()
     for p in _deps():
-        with open(p, "rb") as f:
-            h.update(f.read())
+        if p.endswith(".py"):
+            continue
+        with open(p, "r") as f:
+            h.update(_code_only(f.read()).encode())
+    h.update(repr((NVCC_FLAGS[:-1], FAMILIES)).encode())   # the last flag is the include path of this checkout
     return h.hexdigest()[:16]
 
 
