@@ -42,6 +42,8 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-marginal kernels (<= 102 registers)
 constexpr int kMinPoints = 640;           // smallest point buffer
+constexpr int kMinCtasPerSm = 8, kMaxCtasPerSm = 16;   // CTAs per SM over the whole launch
+constexpr double kPointFoldsPerCta = 2.0e7;            // work per CTA the plan aims for
 
 size_t search_smem_fixed() {  // mbarriers, seg row, Eq. 5 accumulators, the warps' top-k lists + thresholds, light-curve scalars
     return sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) + sizeof(uint64_t) * kMaxWarps * kStatWords +
@@ -122,8 +124,15 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     p.smem = (size_t)(cap + 2) * sizeof(double2) + search_smem_fixed() + (size_t)planes;
     const int64_t tile = (int64_t)p.nt * p.R;
     p.tiles_per_lc = n_trials > 0 ? (n_trials + tile - 1) / tile : 0;
-    // ~16 CTAs per SM overall for dynamic balance, at least one tile per job
-    int64_t want = (148LL * 16 + (n_lc > 0 ? n_lc : 1) - 1) / (n_lc > 0 ? n_lc : 1);
+    // CTAs over the whole launch: enough for dynamic balance at the tail, few enough that a CTA's set-up (zeroing its
+    // counters, staging the light curve, merging its top-k) stays small against its work -- about 2e7 point-folds per
+    // CTA, between 8 and 16 CTAs per SM (measured: C4 9.14 -> 9.03 ms from 16 to 8 per SM; C5 indifferent between 8 and
+    // 64 except 48: +1.3 %); at least one tile per job
+    const int64_t lcs = n_lc > 0 ? n_lc : 1;
+    int64_t ctas = (int64_t)((double)total_points * (double)n_trials / kPointFoldsPerCta);
+    if (ctas < 148LL * kMinCtasPerSm) ctas = 148LL * kMinCtasPerSm;
+    if (ctas > 148LL * kMaxCtasPerSm) ctas = 148LL * kMaxCtasPerSm;
+    int64_t want = (ctas + lcs - 1) / lcs;
     if (want > p.tiles_per_lc) want = p.tiles_per_lc;
     if (want < 1) want = 1;
     if (want > 4096) want = 4096;
