@@ -136,6 +136,17 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     if (want > p.tiles_per_lc) want = p.tiles_per_lc;
     if (want < 1) want = 1;
     if (want > 4096) want = 4096;
+    // One CTA per SM at a time and CTAs of about equal length: the launch takes ceil(CTAs / 148) rounds, so a CTA count
+    // just above a multiple of 148 wastes most of its last round (P1: 100 light curves x 24 jobs = 16.2 rounds).  Up to
+    // twice the jobs are taken when that fills the last round better.
+    auto fill = [&](int64_t j) {
+        const double rounds = (double)(lcs * j) / 148.0;
+        return rounds / ceil(rounds);
+    };
+    int64_t best = want;
+    for (int64_t j = want + 1; j <= 2 * want && j <= p.tiles_per_lc && j <= 4096; ++j)
+        if (fill(j) > fill(best) + 1e-9) best = j;
+    want = best;
     p.jobs_per_lc = (int)want;
     return p;
 }
