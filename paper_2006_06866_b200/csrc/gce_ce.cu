@@ -245,7 +245,7 @@ int dispatch_search(const SearchParams &sp, const Plan &plan, bool dump, int32_t
 // ================================================================================================ C ABI
 extern "C" {
 
-const char *gce_ce_version(void) { return "gce-b200 0.2 (sm_100a)"; }
+const char *gce_ce_version(void) { return "gce-b200 0.3 (sm_100a)"; }
 
 const char *gce_ce_strerror(int code) {
     switch (code) {
