@@ -32,7 +32,8 @@
  * with closed-form CE (0, ln 2, 1/2 ln 2, 0.6059391565991873), scipy.stats.entropy identity
  * H(m,phi) - H(phi), exact rational refold, Eq. 6 closed form, numpy.histogram marginals,
  * invariants 0 <= CE <= H(m), noiseless recovery; N2 overlap: hand tables, exact-rational interval
- * membership, CE_plain <= CE_overlap <= CE_plain + ln 2.  Parity with a CE value printed in the
+ * membership, CE_plain <= CE_overlap <= CE_plain + ln 2; S0 normalisation: hand closed forms, numpy.median /
+ * numpy.std per filter, one-filter bin invariance, a two-filter merged light curve.  Parity with a CE value printed in the
  * paper: UNPINNED (the paper prints none).
  */
 #include <math.h>
