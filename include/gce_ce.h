@@ -52,6 +52,8 @@ extern "C" {
 #define GCE_CE_ERR_RANGE (-2)     /* a size or bin count is out of range                           */
 #define GCE_CE_ERR_WORKSPACE (-3) /* workspace too small or misaligned                             */
 #define GCE_CE_ERR_CUDA (-4)      /* a CUDA runtime call failed; see gce_ce_last_cuda_error()       */
+#define GCE_CE_ERR_STATIC_LIMIT (-5) /* gce_ce_search_static only: the call needs more scratch than
+                                      * GCE_CE_STATIC_SCRATCH_BYTES; use gce_ce_search with a workspace */
 
 #define GCE_CE_MAX_BINS 64         /* n_phase_bins and n_mag_bins are each in 1..64                 */
 #define GCE_CE_MAX_TOPK 32         /* top_k is in 0..32                                             */
@@ -112,6 +114,47 @@ int gce_ce_search(const double *times, const double *mags, const int64_t *lc_off
                   int64_t n_pdot, const gce_ce_params *prm_host, void *out_ce, int64_t *out_best_idx,
                   float *out_best_ce, double *out_stats, void *workspace, size_t workspace_bytes,
                   void *stream);
+
+/*
+ * The same search for callers that cannot allocate device memory at all.
+ *
+ * Who this is for: code that runs as a guest inside somebody else's GPU process -- a survey alert broker, an
+ * acquisition daemon, a plug-in of a pipeline that reserved the whole card for its own pool at start-up.  Such a host
+ * hands the guest input and output buffers and a stream, but no allocator; cudaMalloc is off limits there because it
+ * stalls every stream of the device while it runs, and because it can fail long after start-up once the host has claimed
+ * the memory.  gce_ce_search still needs a workspace from somebody; this entry point needs none.
+ *
+ * How: the scratch memory (grouped points, magnitude-bin segments, the k ln k table, the per-CTA top-k and Eq. 5
+ * partials) lives in an array of GCE_CE_STATIC_SCRATCH_BYTES that is compiled into the library's device image.  Every
+ * GPU on which the library gets loaded carries that array from load until the process exits, whether or not this entry
+ * point is ever called.  The call itself runs no cudaMalloc, no cudaFree and no other routine that allocates: it looks
+ * up the array's device address (first call on each device, see below), checks the sizes and enqueues the same kernels,
+ * in the same launch configuration, as gce_ce_search -- the results are the same bits.
+ *
+ * Arguments, layouts, return codes and stream semantics are those of gce_ce_search, minus workspace / workspace_bytes.
+ * One more return code: GCE_CE_ERR_STATIC_LIMIT when gce_ce_workspace_bytes(total_points, n_lc, n_p, n_pdot, prm) for this
+ * call exceeds GCE_CE_STATIC_SCRATCH_BYTES (nothing is enqueued; the caller can make the same comparison up front).  For
+ * scale: 16 bytes per point, 8 bytes per k ln k entry (at most 65 536 entries without max_lc_points), and 16 * top_k + 64
+ * bytes per CTA of the search launch.  All five BASELINE.json configs fit (C3: 64 000 points, 1.5 MiB; C4: 200 000 points
+ * in 1000 light curves, 3.8 MiB; C5: 2.3 MiB), as does the paper's production grid; a batch of about 450 000 points is
+ * where the limit is reached.
+ *
+ * Set-up: the first call on each device, made with that device current, asks the runtime for the array's address
+ * (cudaGetSymbolAddress; this may load the library's device code on that device) and remembers it.  Make that first
+ * call before the stream is put into capture mode.  Later calls on the device only read the remembered address.
+ *
+ * Sharing: there is ONE array per device and process.  Every call on that device uses it, whatever the stream or host
+ * thread, and it keeps the previous call's contents.  Nothing in it has to start at zero -- each call writes every word
+ * before it reads it -- so no clearing is done or needed.  But two calls whose kernels can be on the GPU at the same time
+ * (different streams without an ordering between them, or two host threads on one device) overwrite each other's
+ * scratch and both return garbage: order them yourself (same stream, or events).  Calls on different devices, and
+ * gce_ce_search calls with their own workspaces, do not interfere.
+ */
+#define GCE_CE_STATIC_SCRATCH_BYTES (8u << 20)
+int gce_ce_search_static(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                         int64_t total_points, const double *periods, int64_t n_p, const double *pdots,
+                         int64_t n_pdot, const gce_ce_params *prm_host, void *out_ce, int64_t *out_best_idx,
+                         float *out_best_ce, double *out_stats, void *stream);
 
 /* Same call with HOST buffers for every array: allocates device memory, copies inputs in, runs the
  * search, copies the requested outputs back and synchronises.  Convenience / end-to-end timing entry. */

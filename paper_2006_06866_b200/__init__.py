@@ -13,6 +13,7 @@ _BINDING_NAMES = (
     "gce_ce_launch_count", "gce_ce_search", "gce_ce_search_host", "gce_ce_validate_host", "gce_ce_version",
     "gce_ce_workspace_bytes", "make_params", "search", "gce_ce_partial_words", "gce_ce_search_partial",
     "gce_ce_merge_partials", "search_period_chunks", "gce_ce_host_release", "gce_ce_probe_rate",
+    "gce_ce_search_static", "STATIC_SCRATCH_BYTES", "ERR_STATIC_LIMIT",
 )
 
 

@@ -23,6 +23,8 @@ _lib = C.CDLL(LIB)
 
 MAX_BINS, MAX_TOPK, MAX_POINTS, MAX_POINTS_OVERLAP, MAX_POINTS_WIDE = 64, 32, 65535, 32767, 1 << 26
 OK, ERR_POINTER, ERR_RANGE, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
+ERR_STATIC_LIMIT = -5                 # gce_ce_search_static: the call needs more than STATIC_SCRATCH_BYTES of scratch
+STATIC_SCRATCH_BYTES = 8 << 20        # GCE_CE_STATIC_SCRATCH_BYTES
 FOLD_AUTO, FOLD_PLAIN, FOLD_PAIR, FOLD_QUAD, FOLD_GENERIC, FOLD_PDOT_ZERO = range(6)   # gce_ce_debug_bins fold_mode
 
 
@@ -37,6 +39,9 @@ _vp, _i32, _i64, _sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
 _lib.gce_ce_workspace_bytes.argtypes = [_i64, _i32, _i64, _i64, C.POINTER(Params), C.POINTER(_sz)]
 _lib.gce_ce_search.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params),
                                _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.gce_ce_search_static.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params),
+                                      _vp, _vp, _vp, _vp, _vp]
+_lib.gce_ce_search_static.restype = C.c_int
 _lib.gce_ce_search_host.argtypes = [_vp, _vp, _vp, _i32, _vp, _i64, _vp, _i64, C.POINTER(Params), _vp, _vp, _vp, _vp]
 _lib.gce_ce_debug_histogram.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp, _i64, _vp, _i64, C.POINTER(Params),
                                         _vp, _i64, _vp, _vp, _vp, _sz, _vp]
@@ -64,7 +69,8 @@ for _f in ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce
 EXPORTS = ("gce_ce_workspace_bytes", "gce_ce_search", "gce_ce_search_host", "gce_ce_debug_histogram",
            "gce_ce_debug_bins", "gce_ce_validate_host", "gce_ce_launch_count", "gce_ce_strerror",
            "gce_ce_last_cuda_error", "gce_ce_version", "gce_ce_partial_words", "gce_ce_search_partial",
-           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release", "gce_ce_probe_rate")
+           "gce_ce_merge_partials", "gce_ce_merge_partials_to_partial", "gce_ce_host_release", "gce_ce_probe_rate",
+           "gce_ce_search_static")
 
 
 class GceError(RuntimeError):
@@ -158,6 +164,37 @@ def gce_ce_search(times, mags, lc_offsets, periods, pdots, prm: Params, out_ce=N
                               periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), _ptr(out_ce),
                               _ptr(out_best_idx), _ptr(out_best_ce), _ptr(out_stats), _ptr(workspace),
                               workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def gce_ce_search_static(times, mags, lc_offsets, periods, pdots, prm: Params, out_ce=None, out_best_idx=None,
+                         out_best_ce=None, out_stats=None, stream=None):
+    """gce_ce_search without a workspace argument, for callers that are not allowed to allocate device memory.
+
+    Meant for code that is a guest in another program's GPU process (an alert broker, a pipeline plug-in): the host
+    program passes in input and output tensors and a stream but owns all the memory, and cudaMalloc is ruled out there
+    because it stalls the whole device and can fail once the host has taken the card's memory.  The scratch the search
+    needs sits in an 8 MiB array (STATIC_SCRATCH_BYTES) built into libgce_ce.so, so this call -- the wrapper included --
+    creates no tensor and the library calls no allocator.  Same kernels, same results as gce_ce_search.
+
+    Raises GceError with code ERR_STATIC_LIMIT (nothing enqueued) when gce_ce_workspace_bytes(...) for these sizes is
+    larger than STATIC_SCRATCH_BYTES.  The first call on a device looks up the array's address; make it before any
+    stream capture starts.  All calls on a device share the one array: calls that can run on the GPU at the same time
+    (unordered streams, several threads) corrupt each other, so keep them ordered on one stream or with events."""
+    times, mags = _dev(times, torch.float64), _dev(mags, torch.float64)
+    lc_offsets = _dev(lc_offsets, torch.int64)
+    periods, pdots = _dev(periods, torch.float64), _dev(pdots, torch.float64)
+    n_lc = lc_offsets.numel() - 1
+    _dev(out_ce, torch.float64 if prm.ce_fp64 else torch.float32)
+    _dev(out_best_idx, torch.int64)
+    _dev(out_best_ce, torch.float32)
+    _dev(out_stats, torch.float64)
+    for t, n, what in ((out_ce, n_lc * periods.numel() * pdots.numel(), "out_ce"), (out_best_idx, n_lc * prm.top_k, "out_best_idx"),
+                       (out_best_ce, n_lc * prm.top_k, "out_best_ce"), (out_stats, n_lc * 4, "out_stats")):
+        if t is not None and t.numel() != n:
+            raise ValueError(f"{what} has the wrong number of elements")
+    _check(_lib.gce_ce_search_static(_ptr(times), _ptr(mags), _ptr(lc_offsets), n_lc, times.numel(), _ptr(periods),
+                                     periods.numel(), _ptr(pdots), pdots.numel(), C.byref(prm), _ptr(out_ce),
+                                     _ptr(out_best_idx), _ptr(out_best_ce), _ptr(out_stats), _stream(stream)))
 
 
 def gce_ce_host_release() -> None:

@@ -254,6 +254,7 @@ const char *gce_ce_strerror(int code) {
         case GCE_CE_ERR_RANGE: return "size, bin count, light-curve length or option out of range";
         case GCE_CE_ERR_WORKSPACE: return "workspace too small or misaligned";
         case GCE_CE_ERR_CUDA: return "CUDA runtime error (see gce_ce_last_cuda_error)";
+        case GCE_CE_ERR_STATIC_LIMIT: return "call needs more scratch than GCE_CE_STATIC_SCRATCH_BYTES (use gce_ce_search with a workspace)";
         default: return "unknown error code";
     }
 }
@@ -393,6 +394,65 @@ int gce_ce_search(const double *times, const double *mags, const int64_t *lc_off
                   void *workspace, size_t workspace_bytes, void *stream) {
     return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, out_ce,
                       out_best_idx, out_best_ce, out_stats, nullptr, 0, nullptr, nullptr, 0, nullptr, workspace, workspace_bytes, stream);
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ gce_ce_search_static
+// Scratch of the entry point for callers that may not allocate (guests of another program's GPU process: no allocator
+// handed to them, cudaMalloc banned because it stalls the device and may fail late; see include/gce_ce.h).  The array is
+// part of this translation unit's device image: every GPU that loads the library holds these 8 MiB until the process
+// exits.  In HOST code the name below is only the handle the runtime registered for the symbol -- it is not a device
+// address and must never be passed to a kernel (the kernel would fault, or where the GPU can reach host memory, quietly
+// work on the wrong bytes).  Host code gets the device address once per device from cudaGetSymbolAddress, with that
+// device current, and passes THAT pointer on.
+static __device__ __align__(256) unsigned char g_static_scratch[GCE_CE_STATIC_SCRATCH_BYTES];
+
+namespace {
+std::mutex g_static_mutex;
+void *g_static_addr[64] = {};  // device address of g_static_scratch on each device, 0 = not looked up yet
+
+// Device address of the scratch array on the current device; the first call per device does the look-up.
+cudaError_t static_scratch_addr(void **addr) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return cudaErrorInvalidSymbol;
+        g_static_addr[dev] = p;
+    }
+    *addr = g_static_addr[dev];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" {
+
+// No cudaMalloc / cudaFree / pool call anywhere below: size checks on the host, one address look-up, then run_search,
+// which only launches kernels and records the caller's events.  The scratch is shared by every call on the device and
+// is not cleared: each call writes what it later reads (the existing path runs on uninitialised workspaces too).
+int gce_ce_search_static(const double *times, const double *mags, const int64_t *lc_offsets, int32_t n_lc,
+                         int64_t total_points, const double *periods, int64_t n_p, const double *pdots, int64_t n_pdot,
+                         const gce_ce_params *prm, void *out_ce, int64_t *out_best_idx, float *out_best_ce,
+                         double *out_stats, void *stream) {
+    int rc = check_params(prm);
+    if (rc) return rc;
+    rc = check_sizes(n_lc, total_points, n_p, n_pdot);
+    if (rc) return rc;
+    if (total_points > (int64_t)n_lc * points_limit(prm)) return GCE_CE_ERR_RANGE;  // some light curve is too long (as in run_search)
+    if (make_layout(total_points, n_lc, n_p * n_pdot, n_pdot, prm).total > (size_t)GCE_CE_STATIC_SCRATCH_BYTES)
+        return GCE_CE_ERR_STATIC_LIMIT;
+    void *scratch = nullptr;
+    const cudaError_t e = static_scratch_addr(&scratch);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, out_ce, out_best_idx,
+                      out_best_ce, out_stats, nullptr, 0, nullptr, nullptr, 0, nullptr, scratch,
+                      (size_t)GCE_CE_STATIC_SCRATCH_BYTES, stream);
 }
 
 size_t gce_ce_partial_words(int32_t top_k) { return (size_t)partial_words(top_k < 0 ? 0 : top_k); }
