@@ -85,7 +85,11 @@ typedef struct gce_ce_params {
     void *ev_search_begin;
     void *ev_search_end;
     /* normalise = 1 only: int32[total_points], the filter (0 .. GCE_CE_MAX_FILTERS - 1) of every point; NULL = all points
-     * belong to one filter.  A DEVICE pointer for the device-pointer calls, a HOST pointer for the *_host calls. */
+     * belong to one filter.  A DEVICE pointer for the device-pointer calls, a HOST pointer for the *_host calls.  An id
+     * outside 0 .. GCE_CE_MAX_FILTERS - 1 is refused (GCE_CE_ERR_RANGE) by gce_ce_search_host and gce_ce_validate_host,
+     * which see the array; on the device-pointer calls it is undefined behaviour like the other device-side values
+     * (the kernel uses the low three bits).  Cost of normalise = 1: sequential sums are part of the frozen arithmetic,
+     * so one thread per filter walks each light curve -- negligible at 1e3 points, seconds near GCE_CE_MAX_POINTS_WIDE. */
     const int32_t *filter_ids;
 } gce_ce_params;
 
@@ -241,7 +245,8 @@ int gce_ce_validate_host(const double *times_host, const double *mags_host, cons
  * enqueues for these arguments (for launch accounting). */
 int gce_ce_launch_count(int32_t n_lc, int64_t n_p, const gce_ce_params *prm_host, int partial);
 
-/* Diagnostic, synchronous: measures on the current device the per-SM issue rate a roofline denominator assumes, with a
+/* Diagnostic, not part of the search ABI and excluded from its stability promise (bench.py uses it to confirm the
+ * roofline denominators; it allocates with cudaMalloc and synchronises).  Measures on the current device the per-SM issue rate a roofline denominator assumes, with a
  * probe kernel of 1024 threads per SM timed by the SM's own clock counter (so the figure is per clock, whatever the
  * clock).  GCE_CE_PROBE_FP64: FP64 lane-operations per SM per clock from independent DADD / DMUL chains (nominal 64 on
  * B200).  GCE_CE_PROBE_SHARED: shared-memory wavefronts per SM per clock from conflict-free RED.shared (nominal 1). */

@@ -44,6 +44,11 @@ constexpr int kMaxThreadsSmemMarg = 640;  // launch bound of the shared-memory-m
 constexpr int kMinPoints = 640;           // smallest point buffer
 constexpr int kMinCtasPerSm = 8, kMaxCtasPerSm = 16;   // CTAs per SM over the whole launch
 constexpr double kPointFoldsPerCta = 2.0e7;            // work per CTA the plan aims for
+// SMs of the B200 the launch plan is tuned for.  Deliberately a constant, not a device query: the plan (and with it the
+// workspace layout and the split of the partial sums) is decided from the sizes alone, so that gce_ce_workspace_bytes
+// needs no device and every GPU gives the same CTA split.  On a part with another SM count the results stay the same
+// and only the fill of the last round of CTAs degrades.
+constexpr int64_t kNumSms = 148;
 
 size_t search_smem_fixed() {  // mbarriers, seg row, Eq. 5 accumulators, the warps' top-k lists + thresholds, light-curve scalars
     return sizeof(uint64_t) * 2 + sizeof(int) * (GCE_CE_MAX_BINS + 4) + sizeof(uint64_t) * kMaxWarps * kStatWords +
@@ -62,13 +67,17 @@ int64_t narrow_limit(const gce_ce_params *prm) { return prm->overlap ? GCE_CE_MA
 bool is_wide(const gce_ce_params *prm) { return (int64_t)prm->max_lc_points > narrow_limit(prm); }
 int64_t points_limit(const gce_ce_params *prm) { return is_wide(prm) ? (int64_t)prm->max_lc_points : narrow_limit(prm); }
 
-// Fixed-point shift of the k ln k table: 2^-42 for tables of up to 2^17 entries (every narrow call), else the largest
-// shift that keeps L(k_max) -- and with it every sum of table entries of one trial, which is at most L(k_max) -- below 2^61.
+// Fixed-point shift of the k ln k table: 2^-42 for tables within the 16-bit counter range (every narrow call: k_max <=
+// 65535), else the largest shift, at most 42, that keeps L(k_max) -- and with it every sum of table entries of one trial,
+// which is at most L(k_max) -- below 2^61.  Eq. 5 needs more than S < 2^61: a warp adds up to 128 squares of d = S - K
+// in 128 bits, so |d| <= max(S, K) must stay below 2^60.5.  S and K are at most mult * N * ln(n_m) * 2^shift with
+// ln(n_m) <= ln 64 = 4.16: narrow calls reach 65535 * 4.16 * 2^42 < 2^60.1, and beyond the 16-bit range ln(k_max) > 11.09,
+// so N ln(n_m) 2^shift < L(k_max) 2^shift * 4.16 / 11.09 < 2^59.6.
 int table_shift(int64_t ltab_n) {
     const double kmax = (double)(ltab_n - 1);
-    if (kmax <= 131070.0) return kLfixShift;
+    if (kmax <= (double)GCE_CE_MAX_POINTS) return kLfixShift;
     const int bits = (int)ceil(log2(kmax * log(kmax)));
-    return 61 - bits;
+    return 61 - bits < kLfixShift ? 61 - bits : kLfixShift;
 }
 
 // Trials per thread and whether they share a period: from the grid shape alone (also used by gce_ce_debug_bins).
@@ -130,17 +139,17 @@ Plan make_plan(int32_t n_lc, int64_t total_points, int64_t n_trials, int64_t n_p
     // 64 except 48: +1.3 %); at least one tile per job
     const int64_t lcs = n_lc > 0 ? n_lc : 1;
     int64_t ctas = (int64_t)((double)total_points * (double)n_trials / kPointFoldsPerCta);
-    if (ctas < 148LL * kMinCtasPerSm) ctas = 148LL * kMinCtasPerSm;
-    if (ctas > 148LL * kMaxCtasPerSm) ctas = 148LL * kMaxCtasPerSm;
+    if (ctas < kNumSms * kMinCtasPerSm) ctas = kNumSms * kMinCtasPerSm;
+    if (ctas > kNumSms * kMaxCtasPerSm) ctas = kNumSms * kMaxCtasPerSm;
     int64_t want = (ctas + lcs - 1) / lcs;
     if (want > p.tiles_per_lc) want = p.tiles_per_lc;
     if (want < 1) want = 1;
     if (want > 4096) want = 4096;
-    // One CTA per SM at a time and CTAs of about equal length: the launch takes ceil(CTAs / 148) rounds, so a CTA count
-    // just above a multiple of 148 wastes most of its last round (P1: 100 light curves x 24 jobs = 16.2 rounds).  Up to
+    // One CTA per SM at a time and CTAs of about equal length: the launch takes ceil(CTAs / kNumSms) rounds, so a CTA count
+    // just above a multiple of kNumSms wastes most of its last round (P1: 100 light curves x 24 jobs = 16.2 rounds).  Up to
     // twice the jobs are taken when that fills the last round better.
     auto fill = [&](int64_t j) {
-        const double rounds = (double)(lcs * j) / 148.0;
+        const double rounds = (double)(lcs * j) / (double)kNumSms;
         return rounds / ceil(rounds);
     };
     int64_t best = want;
@@ -318,6 +327,10 @@ static int run_search(const double *times, const double *mags, const int64_t *lc
     if (n_lc == 0) return GCE_CE_OK;
 
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (dump && n_dump > 0) {  // the dump kernels only write the cells that hold points; first launch-side effect of the call
+        cudaError_t em = cudaMemsetAsync(out_counts, 0, sizeof(uint32_t) * (size_t)n_lc * (size_t)n_dump * prm->n_phase_bins * prm->n_mag_bins, st);
+        if (em != cudaSuccess) return cuda_fail(em);
+    }
     unsigned char *ws = reinterpret_cast<unsigned char *>(workspace);
     double2 *pts = reinterpret_cast<double2 *>(ws + L.pts);
     int32_t *seg = reinterpret_cast<int32_t *>(ws + L.seg);
@@ -525,14 +538,6 @@ int gce_ce_debug_histogram(const double *times, const double *mags, const int64_
                            uint32_t *out_counts, double *out_ce_at, void *workspace, size_t workspace_bytes,
                            void *stream) {
     if (!out_counts) return GCE_CE_ERR_POINTER;
-    int rc = check_params(prm);
-    if (rc) return rc;
-    if (n_lc > 0 && n_trials > 0) {
-        cudaError_t e = cudaMemsetAsync(out_counts, 0,
-                                        sizeof(uint32_t) * (size_t)n_lc * (size_t)n_trials * prm->n_phase_bins * prm->n_mag_bins,
-                                        reinterpret_cast<cudaStream_t>(stream));
-        if (e != cudaSuccess) return cuda_fail(e);
-    }
     return run_search(times, mags, lc_offsets, n_lc, total_points, periods, n_p, pdots, n_pdot, prm, nullptr, nullptr,
                       nullptr, nullptr, trial_q, n_trials, out_counts, out_ce_at, 0, nullptr, workspace, workspace_bytes, stream);
 }
@@ -548,7 +553,7 @@ int gce_ce_debug_bins(const double *times, const double *mags, const int64_t *lc
     if (fold_mode < GCE_CE_FOLD_AUTO || fold_mode > GCE_CE_FOLD_PDOT_ZERO) return GCE_CE_ERR_RANGE;
     int R;
     bool share_p;
-    plan_trials(n_pdot, prm->n_phase_bins, &R, &share_p);
+    plan_trials(n_pdot, is_wide(prm) ? 0 : prm->n_phase_bins, &R, &share_p);  // as make_plan: wide calls run the generic family
     SearchParams sp;
     memset(&sp, 0, sizeof(sp));
     sp.periods = periods; sp.pdots = pdots;
@@ -803,6 +808,9 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
     if ((prm->want_stats != 0) != (out_stats != nullptr)) return GCE_CE_ERR_POINTER;
     if ((prm->top_k > 0) != (out_best_idx != nullptr)) return GCE_CE_ERR_POINTER;
     if (out_best_ce && !out_best_idx) return GCE_CE_ERR_POINTER;
+    if (prm->normalise && prm->filter_ids)  // a HOST array here: ids outside 0 .. GCE_CE_MAX_FILTERS - 1 are refused, not masked
+        for (int64_t i = 0; i < total; ++i)
+            if (prm->filter_ids[i] < 0 || prm->filter_ids[i] >= GCE_CE_MAX_FILTERS) return GCE_CE_ERR_RANGE;
     // a cube of at least 64 MB over at least 64 periods: overlap its transfer with the search, 8 chunks
     if (out_ce && n_lc > 0 && total > 0 && n_p >= 64 &&
         (size_t)n_lc * (size_t)n_p * (size_t)n_pdot * (prm->ce_fp64 ? 8 : 4) >= ((size_t)64 << 20))

@@ -18,6 +18,11 @@ __device__ __forceinline__ int64_t ltab_entry(int k, int shift) {
 // (a + b) * 0.5, when the count is even); mean and sum of squares are SEQUENTIAL sums over the filter's points in
 // light-curve order, one rounding per operation (a thread per filter walks the light curve); sd == 0 -> u = 0.
 // One CTA per light curve.  Order statistics by an 8-pass radix select over the order-preserving 64-bit keys.
+// Cost: the sequential sums are part of the contract (they fix the rounding order the oracle also uses), so ONE thread
+// per filter walks the whole light curve twice, and every filter present adds 8 radix passes over the light curve (16
+// when its count is even): O(N) serial work per light curve -- microseconds at the paper's 1e3 points (DESIGN.md section
+// 14), but seconds per call for a wide call near 2^26 points.  The pipelined host entry (large cubes, 8 period chunks)
+// repeats S0 and S1 for each chunk.  For very long normalised light curves, normalise once outside and pass normalise = 0.
 __device__ __forceinline__ unsigned long long order_key(double v) {
     const unsigned long long b = (unsigned long long)__double_as_longlong(v);
     return (b >> 63) ? ~b : (b | 0x8000000000000000ull);

@@ -639,7 +639,7 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     if (!valid[r]) continue;
-                    const int64_t d = S[r] - K;   // |d| <= max(S, K) < 2^61
+                    const int64_t d = S[r] - K;   // |d| <= max(S, K) < 2^60.1 (table_shift, gce_ce.cu)
                     a += d;
                     b += (u128_t)((__int128)d * d);
                     mn = S[r] < mn ? S[r] : mn;
@@ -649,7 +649,7 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                 u128_t au = (u128_t)a;
                 for (int o = 16; o > 0; o >>= 1) {
                     au += shfl_xor_u128(au, o);
-                    b += shfl_xor_u128(b, o);            // <= 32 * R * 2^122 < 2^128
+                    b += shfl_xor_u128(b, o);            // <= 32 * R * 2^120.2 < 2^128
                     const int64_t m2 = __shfl_xor_sync(0xffffffffu, mn, o), m3 = __shfl_xor_sync(0xffffffffu, mx, o);
                     mn = m2 < mn ? m2 : mn;
                     mx = m3 > mx ? m3 : mx;
@@ -658,6 +658,13 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
                 if (lane == 0) stat_add(sstat + (tid >> 5) * kStatWords, cnt, au, b, 0, mn, mx);
             }
         }
+    }
+
+    // Dump mode skips tiles without a listed trial, so a CTA may get here without ever having waited for the bulk copy
+    // its prologue issued; a CTA must not exit with a copy into its own shared memory in flight (the next CTA on the SM
+    // could see the late bytes or the late mbarrier transaction).  Waiting on a phase that has completed returns at once.
+    if constexpr (DUMP) {
+        if (tid == 0 && single && n_chunks > 0 && n_tiles > 0) mbar_wait(&full[0], 0u);
     }
 
     // ---------------- per-CTA Eq. 5 partial sums -> part_stats[lc][job]

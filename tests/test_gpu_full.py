@@ -336,6 +336,29 @@ def test_wide_counters_period_split_is_exact(gce):
     assert torch.equal(whole.stats, split.stats)
 
 
+def test_eq5_sums_of_a_clean_long_light_curve_do_not_wrap(gce, oracle):
+    """The warp-level Eq. 5 reduction adds up to 128 squares of d = S - K in 128 bits, so |d| must stay below 2^60.5.
+    Worst case: a noiseless signal (CE ~ 0, d ~ -K) in a long light curve with 64 magnitude bins (K = N H(m) 2^shift),
+    many Pdots sharing the true period so that all 128 trials of a warp sit at the minimum.  With the table shift at 42
+    for N = 1e5 this K is 2^60.7 and the sum of squares wrapped; the shift of tables beyond the 16-bit range is now
+    chosen from L(k_max) (gce_ce.cu table_shift), K = 2^58.7.  mean / std / min / rho against the oracle's Eq. 5."""
+    n_obs, n_phi, n_m, P = 100000, 64, 64, 611.0
+    rng = np.random.default_rng(77)
+    t = np.sort(rng.uniform(0, 3e7, n_obs))
+    m = np.mod(t / P, 1.0)                       # sawtooth: the magnitude is the phase, H(m) = ln 64, CE ~ 0 at P
+    offs = np.array([0, n_obs], dtype=np.int64)
+    periods = np.array([P, P * 1.37, P, P * 0.71, P, P * 1.11, P, P], dtype=np.float64)   # rows at P: 128 trials near CE = 0
+    pdots = np.linspace(-1e-19, 0.0, 128)        # no measurable drift: every Pdot of a row gives the same low CE
+    ref = oracle.ce_search(t, m, offs, periods, pdots, n_phi, n_m)
+    assert ref[0, 0].max() < 0.3 * np.log(64) and ref[0, 1].min() > 0.8 * np.log(64)
+    res = gce.search(dev(t), dev(m), dev(offs), dev(periods), dev(pdots), n_phi, n_m, top_k=2, want_cube=True,
+                     ce_fp64=True, want_stats=True)
+    torch.cuda.synchronize()
+    assert_ce_close(res.ce.cpu().numpy(), ref, RTOL64)
+    mu, sigma, rho = oracle.significance(ref[0])
+    np.testing.assert_allclose(res.stats[0].cpu().numpy(), [mu, sigma, ref[0].min(), rho], rtol=RTOL_STATS)
+
+
 # ------------------------------------------------------------------------------------------ N1: fused Eq. 5 statistics
 RTOL_STATS = 1e-9   # DESIGN.md section 10: exact integer sums of N*CE*2^42, one fp64 conversion; the per-trial CE values
                     # differ from the oracle's by <= 1e-12 relative, the variance subtraction amplifies that by mean^2/var
