@@ -21,9 +21,20 @@ roofline: the fold+bin+entropy kernel (k_search), timed live with CUDA events re
           wavefronts -- "bound" names the one that binds (the larger fraction), the other is kept in "other_bound"
 cpu_baseline: the oracle (oracle/, as it stands) on this box's host cores over a bounded sample of the workload
 
-N > 1 (torchrun, one process per GPU): light curves are independent, so each rank searches its own batch of
-the same shape (seed offset by rank; weak scaling, no data-path collective); value = all ranks' point-folds /
-max-over-ranks time.  --impl reference times the oracle instead (rank 0 only).
+N > 1 (one process per GPU): started under torchrun the ranks come from the environment; started plainly as
+`python bench.py --gpus N` (no RANK in the environment) bench.py launches the N ranks itself (torch.distributed.run on
+127.0.0.1) and passes their one JSON line through.  Light curves are independent, so there is no data-path collective.
+  --scaling weak   (default) each rank searches its own batch of the config's shape (seed offset by rank);
+                   value = all ranks' point-folds / max-over-ranks time
+  --scaling strong the GIVEN config is partitioned by light curve (sharding.partition_light_curves, balanced by points;
+                   C5: 16 light curves -> 2 per GPU at N = 8), every rank searches its slice, the per-light-curve
+                   selections are gathered and rank 0 checks them against its own search of the whole config; value =
+                   the config's point-folds / max-over-ranks time.  Fewer light curves than GPUs (one deep target): the
+                   period axis is split instead and the per-rank partial blobs are all-gathered and merged exactly
+                   (search_period_chunks; the path's one real exchange step).
+--dry-run stops before CUDA: the ranks rendezvous over gloo, build the workload and the partition, and rank 0 prints the
+plan as one JSON line (tests/test_bench_contract.py runs it with 2 ranks on CPU).
+--impl reference times the oracle instead (rank 0 only).
 """
 from __future__ import annotations
 
@@ -132,6 +143,23 @@ def make_workload(name, rank, shrink, n_pdot=0):
         # weak scaling: every rank owns a batch of the same shape; rank r re-draws it from seed + 1000 r
         kw = dict(kw, seed={"C1": 0, "C2": 1, "C3": 2, "C4": 3, "C5": 4, "P1": 9}[name] + 1000 * rank)
     return W.make(name, **kw)
+
+
+def rank_workload(name, rank, world, args, n_pdot=0):
+    """(this rank's workload, the whole config or None, the light-curve ranges or None).  weak: a batch of the config's
+    shape per rank.  strong: the given config partitioned by light curve."""
+    if args.scaling != "strong" or world == 1:
+        return apply_binning(make_workload(name, rank, args.quick, n_pdot), args), None, None
+    from paper_2006_06866_b200 import sharding
+    full = apply_binning(make_workload(name, 0, args.quick, n_pdot), args)
+    if full.n_lc < world:
+        return full, full, None   # fewer light curves than ranks: the period axis is split instead (measure_period_split)
+    ranges = sharding.partition_light_curves(full.lc_offsets, world)
+    lo, hi = ranges[rank]
+    t, m, offs = sharding.shard_arrays(full.times, full.mags, full.lc_offsets, lo, hi)
+    mine = W.Workload(f"{full.name}[{lo}:{hi}]", t, m, np.ascontiguousarray(offs), full.periods, full.pdots,
+                      full.n_phase_bins, full.n_mag_bins, full.top_k, full.want_cube)
+    return mine, full, ranges
 
 
 def apply_binning(w, args):
@@ -247,7 +275,7 @@ def traffic_record(w, args):
 
 
 # ----------------------------------------------------------------------------------------- our arm
-def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline):
+def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline, keep=None):
     """W warm-ups, K timed steps (device-resident), the end-to-end host-buffer leg, the roofline record; one dict."""
     import torch
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
@@ -323,6 +351,8 @@ def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline)
     e2e_val = pf_all * n_e2e / float(te.item())
     if k and rank == 0:
         assert torch.equal(h_idx.to(dev), bidx), "host and device entry points disagree"
+    if keep is not None and k:
+        keep["best_idx"] = bidx.cpu().numpy()
     del ce, ws, flush, h_ce
     gce.gce_ce_host_release()
     torch.cuda.empty_cache()
@@ -375,12 +405,161 @@ def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline)
                "sample": desc, "seconds": t_cpu}
 
     return {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(w, args),
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
                     "api": "gce_ce_search_host (pinned host buffers; allocation + H2D + search + D2H + sync; with a cube the period "
                            "axis is searched in 8 chunks and each slice's D2H overlaps the next chunk on a second stream)"},
             "gpu_launches": launches_per_step * args.steps, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu}
+
+
+def period_ranges(n_p, world):
+    """Contiguous period ranges [a, b) per rank (the work of a period does not depend on its value for the plain fold)."""
+    return [(n_p * r // world, n_p * (r + 1) // world) for r in range(world)]
+
+
+def measure_period_split(gce, w, args, dev, dist, rank, world, local_rank):
+    """Strong scaling of a config with fewer light curves than GPUs (one deep target): every rank
+    searches all light curves over its slice of the period axis (gce_ce_search_partial), the per-rank partial blobs --
+    n_lc x (2 top_k + 10) int64, the path's one exchange -- are all-gathered (NCCL, in stream order) and merged exactly
+    by every rank (gce_ce_merge_partials).  A step is that whole sequence; the cube, when the config asks for one, is
+    left sharded by period on the ranks.  No roofline record: k_search is the same kernel the N = 1 line describes."""
+    import torch
+    from paper_2006_06866_b200 import sharding
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    args_dev = (d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots), w.n_phase_bins, w.n_mag_bins)
+    k = max(1, w.top_k)
+    a, b = period_ranges(w.n_p, world)[rank]
+    sink = (lambda lo, hi, sl: None) if w.want_cube else None
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        return gce.search_period_chunks(*args_dev, [(a, b)] if b > a else [], top_k=k, want_stats=False, overlap=args.overlap,
+                                        cube_sink=sink, dist=dist)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sync_all()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    s_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    e_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    sync_all()
+    t0 = time.time()
+    for i in range(args.steps):
+        flush.zero_()
+        s_ev[i].record()
+        res = step()
+        e_ev[i].record()
+    sync_all()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    tot_ms = float(sum(s.elapsed_time(e) for s, e in zip(s_ev, e_ev)))
+    my_pf = float(w.total_points) * (b - a) * w.n_pdot
+    tot_ms_max, pf_all = sharding.reduce_timing(tot_ms, my_pf, dist, dev)
+    if rank != 0:
+        return None
+    whole = gce.search(*args_dev, top_k=k, want_cube=False, overlap=args.overlap)   # the N = 1 selection, outside the timing
+    torch.cuda.synchronize()
+    equal = bool(torch.equal(whole.best_idx, res.best_idx) and torch.equal(whole.best_ce, res.best_ce))
+    assert equal, "period-split selection differs from the single-GPU search"
+    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=k, overlap=args.overlap)
+    cfg = workload_config(w, args)
+    cfg["parallelism"] = f"period axis split x{world}, partial blobs all-gathered ({dist.get_backend()}) and merged exactly"
+    return {"metric": METRIC, "value": pf_all * args.steps / (tot_ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "e2e": None,
+            "gpu_launches": (gce.gce_ce_launch_count(w.n_lc, b - a, prm, partial=True) + 2) * args.steps, "clocks": clocks,
+            "roofline": None, "cpu_baseline": None,
+            "strong_check": {"mode": "period split", "period_ranges": period_ranges(w.n_p, world), "equal_to_single_gpu": equal}}
+
+
+def measure_any(gce, name, args, dev, dist, rank, world, local_rank, with_cpu_baseline, n_pdot=0):
+    """One config in the requested scaling mode; rank 0 gets the record."""
+    import torch
+    from paper_2006_06866_b200 import sharding
+    w, full, ranges = rank_workload(name, rank, world, args, n_pdot)
+    if full is not None and ranges is None:
+        return measure_period_split(gce, full, args, dev, dist, rank, world, local_rank)
+    keep = {} if full is not None else None
+    line = measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline, keep=keep)
+    if full is None:
+        return line
+    # strong scaling by light curve: gather the selections in light-curve order; rank 0 compares with the whole config
+    k = full.top_k
+    if k:
+        local = keep.get("best_idx", np.zeros((0, k), dtype=np.int64))
+        gathered = sharding.gather_per_light_curve(local, full.n_lc, ranges, rank, dist)
+    if rank != 0:
+        return None
+    equal = None
+    if k:
+        d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        whole = gce.search(d(full.times), d(full.mags), d(full.lc_offsets), d(full.periods), d(full.pdots), full.n_phase_bins,
+                           full.n_mag_bins, top_k=k, want_cube=False, overlap=args.overlap)
+        torch.cuda.synchronize()
+        equal = bool(np.array_equal(whole.best_idx.cpu().numpy(), gathered))
+        assert equal, "gathered per-light-curve selections differ from the single-GPU search of the whole config"
+    line["config"] = dict(workload_config(full, args), point_folds_per_step_per_gpu=None, point_folds_per_step=full.point_folds,
+                          parallelism=f"the config's light curves partitioned over {world} GPUs, balanced by points; no data-path collective")
+    line["strong_check"] = {"mode": "light-curve partition", "lc_ranges": ranges, "equal_to_single_gpu": equal}
+    return line
+
+
+def run_dry(args):
+    """--dry-run: everything up to CUDA.  The ranks rendezvous over gloo, build the workload and the partition of the
+    requested scaling mode, and rank 0 prints the plan."""
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("gloo")
+    name = args.config or DEFAULT_CONFIG
+    if name == "P1":
+        args.overlap = True
+        OVERLAP[0] = True
+    w, full, ranges = rank_workload(name, rank, world, args, args.n_pdot)
+    if full is not None and ranges is None:
+        a, b = period_ranges(full.n_p, world)[rank]
+        mine = {"rank": rank, "lc_range": [0, full.n_lc], "period_range": [a, b], "point_folds": full.total_points * (b - a) * full.n_pdot}
+    else:
+        mine = {"rank": rank, "lc_range": list(ranges[rank]) if ranges else [0, w.n_lc], "period_range": [0, w.n_p],
+                "point_folds": w.point_folds, "sha256_16": array_sha256(w)}
+    plans = [mine]
+    if world > 1:
+        plans = [None] * world
+        dist.all_gather_object(plans, mine)
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "n_gpus": world, "scaling": args.scaling, "config": workload_config(full or w, args),
+                          "point_folds_total": sum(p["point_folds"] for p in plans), "ranks": plans}))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def self_launch(args, argv):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks (one process per GPU) and pass their output through."""
+    import socket
+    if not args.dry_run:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            sys.stderr.write(f"bench.py: --gpus {args.gpus} asked for, {have} CUDA device(s) visible; not starting\n")
+            return 2
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+    return subprocess.call(cmd)
 
 
 def run_ours(args):
@@ -409,15 +588,13 @@ def run_ours(args):
     if name == "P1":
         args.overlap = True   # the paper's production binning
         OVERLAP[0] = True
-    w = apply_binning(make_workload(name, rank, args.quick, args.n_pdot), args)
-    line = measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline=not args.no_cpu_baseline)
+    line = measure_any(gce, name, args, dev, dist, rank, world, local_rank, not args.no_cpu_baseline, args.n_pdot)
     if args.config is None:
         # the other P-Pdot grid the north_star's roofline target is stated on, same K / W, its own record
-        w2 = apply_binning(make_workload(SECONDARY_CONFIG, rank, args.quick), args)
-        sec = measure(gce, w2, args, dev, dist, rank, world, local_rank, with_cpu_baseline=False)
+        sec = measure_any(gce, SECONDARY_CONFIG, args, dev, dist, rank, world, local_rank, False)
         if rank == 0:
-            line["secondary"] = {key: sec[key] for key in ("value", "unit", "ms_per_step", "steps", "warmup", "config", "e2e",
-                                                           "gpu_launches", "clocks", "roofline")}
+            line["secondary"] = {key: sec.get(key) for key in ("value", "unit", "ms_per_step", "steps", "warmup", "config", "e2e",
+                                                               "gpu_launches", "clocks", "roofline", "strong_check")}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -488,9 +665,22 @@ def main():
     ap.add_argument("--overlap", action="store_true", help="50 %% overlapping phase bins (N2, PAPER.md:106)")
     ap.add_argument("--n-pdot", type=int, default=0, help="P1 only: 32 / 128 / 512 log-spaced Pdot values (PAPER.md:170)")
     ap.add_argument("--sweep", action="store_true", help="the paper's Fig. 3 sweep instead of the benchmark line")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = a batch of the config's shape per GPU; strong = the given config partitioned over the GPUs")
+    ap.add_argument("--dry-run", action="store_true", help="stop before CUDA: rendezvous (gloo), workload and partition only")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     OVERLAP[0] = bool(args.overlap)
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    in_launcher = "RANK" in os.environ and "WORLD_SIZE" in os.environ
+    if in_launcher and int(os.environ["WORLD_SIZE"]) != args.gpus and args.impl == "ours":
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ['WORLD_SIZE']}; launch one rank per GPU\n")
+        return 2
+    if args.gpus > 1 and not in_launcher and args.impl == "ours" and not args.sweep:
+        return self_launch(args, sys.argv[1:])   # one process per GPU; never a silent single-rank run
+    if args.dry_run:
+        return run_dry(args)
     if args.sweep:
         return run_sweep(args)
     if args.impl == "reference":
