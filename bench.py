@@ -67,9 +67,9 @@ SECONDARY_CONFIG = "C3"            # configs[2]: the other P-Pdot grid of the no
 # (paper_2006_06866_b200.build.source_hash) they were captured from.  C3 writes the 819.2 MB fp32 cube (part of it is
 # still in L2 at kernel end); C5 writes no cube.  Only workloads that were captured have an entry.
 NCU_TRAFFIC = {
-    "C3": {"bytes": 14.615808e6 + 769.364736e6, "source_hash": "8e3b11d7528e880e", "profile": "profiles/r2_k_search_C3_full.md"},
-    "C5": {"bytes": 2.509312e6, "source_hash": "8e3b11d7528e880e", "profile": "profiles/r2_k_search_C5_full.md"},
-    "C4": {"bytes": 4.464896e6, "source_hash": "8e3b11d7528e880e", "profile": "profiles/r2_k_search_C4_full.md"},
+    "C3": {"bytes": 10.908928e6 + 768.851968e6, "source_hash": "a71be253369904fc", "profile": "profiles/r3_k_search_C3_full.md"},
+    "C5": {"bytes": 2.557440e6, "source_hash": "a71be253369904fc", "profile": "profiles/r3_k_search_C5_full.md"},
+    "C4": {"bytes": 4.463616e6, "source_hash": "a71be253369904fc", "profile": "profiles/r3_k_search_C4_full.md"},
 }
 
 
