@@ -602,6 +602,77 @@ def run_ours(args):
     return 0
 
 
+# ----------------------------------------------------------------------------------------- design ablation
+def load_ablation():
+    import ctypes as C
+    from paper_2006_06866_b200.build import build_ablation
+    lib = C.CDLL(build_ablation())
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    lib.gce_ablation_warp_per_trial.argtypes = [vp, vp, vp, i32, i32, vp, i64, vp, i64, i32, i32, vp, C.POINTER(i32), vp]
+    lib.gce_ablation_warp_per_trial.restype = C.c_int
+    return lib
+
+
+def run_ablation(args):
+    """The north_star's histogram sketch (one warp per trial, private 2-D table, match_any-aggregated shared atomics;
+    csrc/gce_ablation.cu, its own shared object) timed beside the product's k_search on the same config, cube output only,
+    same inputs, CUDA events, L2 flushed between steps; the two cubes are compared.  One JSON line."""
+    import ctypes as C
+    import torch
+    from paper_2006_06866_b200.build import build
+    build()
+    import paper_2006_06866_b200 as gce
+    lib = load_ablation()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    w = apply_binning(make_workload(args.config or SECONDARY_CONFIG, 0, args.quick), args)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    t, m, offs, per, pd = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
+    longest = int(np.max(np.diff(w.lc_offsets)))
+    cube_a = torch.empty((w.n_lc, w.n_p, w.n_pdot), dtype=torch.float32, device=dev)
+    cube_p = torch.empty_like(cube_a)
+    prm = gce.make_params(w.n_phase_bins, w.n_mag_bins, top_k=0)
+    ws = torch.empty(gce.gce_ce_workspace_bytes(w.total_points, w.n_lc, w.n_p, w.n_pdot, prm), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    err = C.c_int32(0)
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    def ablation():
+        rc = lib.gce_ablation_warp_per_trial(t.data_ptr(), m.data_ptr(), offs.data_ptr(), w.n_lc, longest, per.data_ptr(), w.n_p,
+                                             pd.data_ptr(), w.n_pdot, w.n_phase_bins, w.n_mag_bins, cube_a.data_ptr(), C.byref(err), st)
+        if rc:
+            raise SystemExit(f"gce_ablation_warp_per_trial failed: {rc} (cudaError {err.value})")
+
+    def product():
+        gce.gce_ce_search(t, m, offs, per, pd, prm, cube_p, None, None, None, ws)
+
+    def timed(fn):
+        for _ in range(args.warmup):
+            fn()
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(args.steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); b.synchronize()
+            ms.append(a.elapsed_time(b))
+        return float(np.mean(ms))
+
+    sampler = ClockSampler(0)
+    sampler.start()
+    t0 = time.time()
+    ms_a, ms_p = timed(ablation), timed(product)
+    clocks = sampler.stop(t0, time.time())
+    rel = float(((cube_a - cube_p).abs() / cube_p.abs().clamp_min(1e-30)).max().item())
+    assert rel < 1e-5, f"the ablation kernel and k_search disagree: max relative difference {rel:.3e}"
+    print(json.dumps({"ablation": "warp per trial, private n_phi x n_m table, match_any-aggregated shared atomics (north_star sketch)",
+                      "config": workload_config(w, args), "steps": args.steps, "warmup": args.warmup, "unit": UNIT,
+                      "ablation_ms": ms_a, "ablation_value": w.point_folds / (ms_a * 1e-3),
+                      "product_ms": ms_p, "product_value": w.point_folds / (ms_p * 1e-3), "product_over_ablation": ms_a / ms_p,
+                      "max_rel_diff_of_the_cubes": rel, "clocks": clocks}))
+    return 0
+
+
 # ----------------------------------------------------------------------------------------- Fig. 3 sweep
 def run_sweep(args):
     """The paper's only timing result (Fig. 3): time per light curve per search point against the
@@ -667,6 +738,8 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="the paper's Fig. 3 sweep instead of the benchmark line")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = a batch of the config's shape per GPU; strong = the given config partitioned over the GPUs")
+    ap.add_argument("--ablation", action="store_true",
+                    help="time the north_star's warp-per-trial / match_any histogram sketch beside k_search (default config C3)")
     ap.add_argument("--dry-run", action="store_true", help="stop before CUDA: rendezvous (gloo), workload and partition only")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -679,6 +752,8 @@ def main():
         return 2
     if args.gpus > 1 and not in_launcher and args.impl == "ours" and not args.sweep:
         return self_launch(args, sys.argv[1:])   # one process per GPU; never a silent single-rank run
+    if args.ablation:
+        return run_ablation(args)
     if args.dry_run:
         return run_dry(args)
     if args.sweep:

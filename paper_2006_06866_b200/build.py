@@ -42,7 +42,7 @@ def _units():
 
 
 def _deps():
-    return [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh"))] + [HDR, os.path.abspath(__file__)]
+    return [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh")) and f != "gce_ablation.cu"] + [HDR, os.path.abspath(__file__)]
 
 
 def _code_only(text: str) -> str:
@@ -102,6 +102,21 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), jobs: int 
     finally:
         shutil.rmtree(obj_dir, ignore_errors=True)
     return LIB
+
+
+ABLATION_LIB = os.path.join(HERE, "libgce_ablation.so")
+
+
+def build_ablation(force: bool = False) -> str:
+    """The design-ablation probe (csrc/gce_ablation.cu: the north_star's warp-per-trial + match_any histogram), its own
+    shared object: bench.py --ablation and its GPU test load it; the product library does not contain it."""
+    src = os.path.join(CSRC, "gce_ablation.cu")
+    if not force and os.path.exists(ABLATION_LIB) and os.path.getmtime(ABLATION_LIB) >= os.path.getmtime(src):
+        return ABLATION_LIB
+    tmp = ABLATION_LIB + f".tmp{os.getpid()}"
+    subprocess.check_call([os.environ.get("NVCC", "nvcc"), *NVCC_FLAGS, "-shared", "-o", tmp, src])
+    os.replace(tmp, ABLATION_LIB)
+    return ABLATION_LIB
 
 
 if __name__ == "__main__":

@@ -53,3 +53,27 @@ def test_probe_rates_are_near_the_nominal_figures():
     assert 55.0 < f < 66.0 and 0.85 < s < 1.05
     with pytest.raises(gce.GceError):
         gce.gce_ce_probe_rate(7)
+
+
+def test_design_ablation_kernel_matches_the_oracle(oracle):
+    """csrc/gce_ablation.cu (the north_star's warp-per-trial + match_any sketch, its own shared object, timed by
+    bench.py --ablation) computes the same CE as the oracle on a small C3-shaped case with a ragged last warp of points."""
+    import ctypes as C
+
+    import numpy as np
+    import torch
+
+    import bench
+    import gce_workloads as W
+    lib = bench.load_ablation()
+    w = W.make("C3", n_lc=3, n_p=257, n_pdot=8)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    t, m, offs, per, pd = d(w.times), d(w.mags), d(w.lc_offsets), d(w.periods), d(w.pdots)
+    out = torch.full((3, 257, 8), -1.0, dtype=torch.float32, device="cuda")
+    err = C.c_int32(0)
+    rc = lib.gce_ablation_warp_per_trial(t.data_ptr(), m.data_ptr(), offs.data_ptr(), 3, int(np.max(np.diff(w.lc_offsets))),
+                                         per.data_ptr(), 257, pd.data_ptr(), 8, 20, 10, out.data_ptr(), C.byref(err), None)
+    torch.cuda.synchronize()
+    assert rc == 0, err.value
+    ref = oracle.ce_search(w.times, w.mags, w.lc_offsets, w.periods, w.pdots, 20, 10)
+    np.testing.assert_allclose(out.cpu().numpy().astype(np.float64), ref, rtol=1e-5, atol=1e-7)
