@@ -67,9 +67,9 @@ SECONDARY_CONFIG = "C3"            # configs[2]: the other P-Pdot grid of the no
 # (paper_2006_06866_b200.build.source_hash) they were captured from.  C3 writes the 819.2 MB fp32 cube (part of it is
 # still in L2 at kernel end); C5 writes no cube.  Only workloads that were captured have an entry.
 NCU_TRAFFIC = {
-    "C3": {"bytes": 10.908928e6 + 768.851968e6, "source_hash": "a71be253369904fc", "profile": "profiles/r3_k_search_C3_full.md"},
-    "C5": {"bytes": 2.557440e6, "source_hash": "a71be253369904fc", "profile": "profiles/r3_k_search_C5_full.md"},
-    "C4": {"bytes": 4.463616e6, "source_hash": "a71be253369904fc", "profile": "profiles/r3_k_search_C4_full.md"},
+    "C3": {"bytes": 15.283456e6 + 769.811456e6, "source_hash": "25ab21d75632df2d", "profile": "profiles/r3_k_search_C3_full.md"},
+    "C5": {"bytes": 2.521600e6, "source_hash": "25ab21d75632df2d", "profile": "profiles/r3_k_search_C5_full.md"},
+    "C4": {"bytes": 4.464640e6, "source_hash": "25ab21d75632df2d", "profile": "profiles/r3_k_search_C4_full.md"},
 }
 
 
@@ -352,7 +352,7 @@ def measure(gce, w, args, dev, dist, rank, world, local_rank, with_cpu_baseline,
     if k and rank == 0:
         assert torch.equal(h_idx.to(dev), bidx), "host and device entry points disagree"
     if keep is not None and k:
-        keep["best_idx"] = bidx.cpu().numpy()
+        keep["best_idx"], keep["best_ce"] = bidx.cpu().numpy(), bce.cpu().numpy()
     del ce, ws, flush, h_ce
     gce.gce_ce_host_release()
     torch.cuda.empty_cache()
@@ -495,8 +495,8 @@ def measure_any(gce, name, args, dev, dist, rank, world, local_rank, with_cpu_ba
     # strong scaling by light curve: gather the selections in light-curve order; rank 0 compares with the whole config
     k = full.top_k
     if k:
-        local = keep.get("best_idx", np.zeros((0, k), dtype=np.int64))
-        gathered = sharding.gather_per_light_curve(local, full.n_lc, ranges, rank, dist)
+        gathered = sharding.gather_per_light_curve(keep.get("best_idx", np.zeros((0, k), dtype=np.int64)), full.n_lc, ranges, rank, dist)
+        gathered_ce = sharding.gather_per_light_curve(keep.get("best_ce", np.zeros((0, k), dtype=np.float32)), full.n_lc, ranges, rank, dist)
     if rank != 0:
         return None
     equal = None
@@ -505,11 +505,18 @@ def measure_any(gce, name, args, dev, dist, rank, world, local_rank, with_cpu_ba
         whole = gce.search(d(full.times), d(full.mags), d(full.lc_offsets), d(full.periods), d(full.pdots), full.n_phase_bins,
                            full.n_mag_bins, top_k=k, want_cube=False, overlap=args.overlap)
         torch.cuda.synchronize()
-        equal = bool(np.array_equal(whole.best_idx.cpu().numpy(), gathered))
-        assert equal, "gathered per-light-curve selections differ from the single-GPU search of the whole config"
+        # A rank's call has fewer points than the whole config's, so its k ln k table may take a finer fixed-point shift
+        # (gce_ce.cu table_shift): the selections agree except, possibly, inside a near tie (north_star's own exception),
+        # where the two CE values are equal to fp32 precision.
+        w_idx, w_ce = whole.best_idx.cpu().numpy(), whole.best_ce.cpu().numpy()
+        differ = w_idx != gathered
+        equal = bool(not differ.any())
+        assert np.allclose(w_ce[differ], gathered_ce[differ], rtol=1e-6, atol=0.0), \
+            "gathered per-light-curve selections differ from the single-GPU search of the whole config"
     line["config"] = dict(workload_config(full, args), point_folds_per_step_per_gpu=None, point_folds_per_step=full.point_folds,
                           parallelism=f"the config's light curves partitioned over {world} GPUs, balanced by points; no data-path collective")
-    line["strong_check"] = {"mode": "light-curve partition", "lc_ranges": ranges, "equal_to_single_gpu": equal}
+    line["strong_check"] = {"mode": "light-curve partition", "lc_ranges": ranges, "equal_to_single_gpu": equal,
+                            "near_tie_differences": int(differ.sum()) if k else 0}
     return line
 
 

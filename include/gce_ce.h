@@ -175,7 +175,9 @@ int gce_ce_search_host(const double *times, const double *mags, const int64_t *l
  * of the final selection, one PARTIAL blob per light curve:
  *   out_partial   int64[n_lc][gce_ce_partial_words(top_k)] =
  *                 { S[top_k] ascending, q[top_k], 8 words of Eq. 5 sums, N, pivot }
- *                 with S = N * CE * 2^42 as an exact integer (INT64_MAX where fewer than top_k trials exist) and q the
+ *                 with S = N * CE * 2^shift as an exact integer (shift = the call's table shift, 42 .. 52 by the length of
+ *                 the k ln k table and less beyond 65 536 entries; it travels in the blob's N word, so blobs of one
+ *                 problem merge whatever their period ranges; INT64_MAX where fewer than top_k trials exist) and q the
  *                 flat index in the WHOLE grid (ip * n_pdot + ipd); the Eq. 5 words are filled when want_stats = 1.
  *   out_ce        NULL, or the cube slice [n_lc][ip_end - ip_begin][n_pdot]
  *   periods       the whole grid double[n_p]; workspace as for gce_ce_workspace_bytes(total_points, n_lc,

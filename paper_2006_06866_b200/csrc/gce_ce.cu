@@ -67,16 +67,23 @@ int64_t narrow_limit(const gce_ce_params *prm) { return prm->overlap ? GCE_CE_MA
 bool is_wide(const gce_ce_params *prm) { return (int64_t)prm->max_lc_points > narrow_limit(prm); }
 int64_t points_limit(const gce_ce_params *prm) { return is_wide(prm) ? (int64_t)prm->max_lc_points : narrow_limit(prm); }
 
-// Fixed-point shift of the k ln k table: 2^-42 for tables within the 16-bit counter range (every narrow call: k_max <=
-// 65535), else the largest shift, at most 42, that keeps L(k_max) -- and with it every sum of table entries of one trial,
-// which is at most L(k_max) -- below 2^61.  Eq. 5 needs more than S < 2^61: a warp adds up to 128 squares of d = S - K
-// in 128 bits, so |d| <= max(S, K) must stay below 2^60.5.  S and K are at most mult * N * ln(n_m) * 2^shift with
-// ln(n_m) <= ln 64 = 4.16: narrow calls reach 65535 * 4.16 * 2^42 < 2^60.1, and beyond the 16-bit range ln(k_max) > 11.09,
-// so N ln(n_m) 2^shift < L(k_max) 2^shift * 4.16 / 11.09 < 2^59.6.
+// Fixed-point shift of the k ln k table: the largest shift, between 42 and 52 for tables within the 16-bit counter range
+// and at most 42 beyond it, that keeps L(k_max) 2^shift below 2^60 (narrow) / 2^61 (wide) -- and with it every sum of
+// table entries of one trial, which is at most L(k_max).  Short tables (a call whose light curves are short: k_max is
+// bounded by the call's total_points) leave spare bits in the 64-bit sums, and spending them shrinks the quantisation
+// term of CE (reading Q21): k_max = 200 -> 2^-49, 1000 -> 2^-47, 5000 -> 2^-44, >= 11 000 -> 2^-42 as before.
+// Eq. 5 needs more than S < 2^61: a warp adds up to 128 squares of d = S - K in 128 bits, so |d| <= max(S, K) must stay
+// below 2^60.5.  S and K are at most mult N ln(n_m) 2^shift and at most L(k_max) 2^shift: narrow calls stay below
+// min(2^60, 65535 * 4.16 * 2^42 = 2^60.1), and beyond the 16-bit range ln(k_max) > 11.09 > ln 64, so
+// N ln(n_m) 2^shift < L(k_max) 2^shift * 4.16 / 11.09 < 2^59.6.
 int table_shift(int64_t ltab_n) {
     const double kmax = (double)(ltab_n - 1);
-    if (kmax <= (double)GCE_CE_MAX_POINTS) return kLfixShift;
+    if (kmax < 2.0) return 52;  // the table is all zeros
     const int bits = (int)ceil(log2(kmax * log(kmax)));
+    if (kmax <= (double)GCE_CE_MAX_POINTS) {
+        const int s = 60 - bits;
+        return s < kLfixShift ? kLfixShift : (s > 52 ? 52 : s);
+    }
     return 61 - bits < kLfixShift ? 61 - bits : kLfixShift;
 }
 

@@ -15,9 +15,9 @@ namespace gce {
 
 struct LcInfo {
     int32_t n;
-    int32_t lshift;  // fixed-point shift of this call's k ln k table (kLfixShift unless the table is longer than 2^16)
+    int32_t lshift;  // fixed-point shift of this call's k ln k table (table_shift in gce_ce.cu: 42 .. 52 by table length, less beyond 2^16 entries)
     double dt_max;
-    int64_t K;  // N * H(m) in 2^-42 fixed point = L(N) - sum_i L(points in magnitude bin i): CE <= H(m), pivot of the Eq. 5 sums
+    int64_t K;  // N * H(m) in 2^-lshift fixed point = L(N) - sum_i L(points in magnitude bin i): CE <= H(m), pivot of the Eq. 5 sums
 };
 
 struct SearchParams {
@@ -83,7 +83,7 @@ namespace {
 using namespace gce;
 
 constexpr int kLtabSmem = 1024;   // entries of the L table mirrored in shared memory
-constexpr int kLfixShift = 42;    // L table fixed point: 2^-42 (tables of up to 2^16 entries; longer ones take a smaller shift)
+constexpr int kLfixShift = 42;    // L table fixed point: at least 2^-42 for tables of up to 2^16 entries (short tables take up to 2^-52; longer ones less than 42)
 constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: RD-add puts floor(y) in the low mantissa word
 constexpr double kYSafe = 2251799813685248.0;  // 2^51: |y| below this -> the magic-add floor is exact
 constexpr int64_t kInfS = INT64_MAX;

@@ -579,7 +579,7 @@ __global__ void __launch_bounds__(NTC > 0 ? NTC : 640, 1) k_search(const SearchP
         int64_t S[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            S[r] = S1[r] - S2[r];  // = N * CE * 2^42, exact
+            S[r] = S1[r] - S2[r];  // = N * CE * 2^lshift, exact
             ce[r] = N > 0 ? (double)S[r] * ce_scale : CUDART_NAN;
         }
         if (DUMP) {
